@@ -526,24 +526,31 @@ def test_breaking_inactive_is_bit_identical_and_nu_nonnegative(O):
 
 
 def test_breaking_dissipates_on_steep_front_only(O):
-    # steep forward-facing front: div q << 0 -> B > 1 -> nu > 0 (eq. (9)); on a sloping bed the
-    # source 2 nu u_x grad(H) changes q and w; mass is untouched; flat bed => q source vanishes.
+    # steep forward-facing front: div q << 0 -> B > 1 -> nu > 0 (eq. (9)): the source R_w = 2 nu
+    # div(u) acts on w (and through the elliptic solve on p, q); mass is untouched.  The mirrored,
+    # rear-facing front has div q >= U1 > 0 -> B = 1 - div q/U1 <= 0 -> nu = 0 (L136-143): the
+    # result is bit-identical to breaking off (P12).
     nx, ny, dx = 128, 4, 0.05
     x = (np.arange(nx) + 0.5) * dx
     for slope in (0.0, 0.05):
         H = np.tile(0.5 - slope * (x - 3.2), (ny, 1))
-        eta = 0.25 * 0.5 * (1 - np.tanh((x - 3.2) / 0.08))
-        h = H + eta[None, :]
-        u = 2.0 * eta / 0.25
-        st = {}
-        for br in (0, 1):
-            o = O.Oracle(nx, ny, dx, 1e3, H, breaking=br, B1=0.15, B2=0.5,
-                         bc_xlo=OUT, bc_xhi=OUT, bc_ylo=PER, bc_yhi=PER)
-            o.set_state(h, h * u[None, :], 0 * h)
-            o.nonhydro_correct(1e-3)
-            st[br] = o.get_state()
-        assert np.array_equal(st[0]["h"], st[1]["h"])
-        dw = st[1]["w"] - st[0]["w"]
-        assert np.abs(dw).max() > 1e-6                       # R_w = 2 nu div(u) acted
-        far = np.abs(x - 3.2) > 1.0
-        assert np.abs(st[1]["qx"] - st[0]["qx"])[:, far].max() < 1e-12   # nu = 0 away from the front
+        for facing in (+1, -1):
+            eta = 0.25 * 0.5 * (1 - facing * np.tanh((x - 3.2) / 0.08))
+            h = H + eta[None, :]
+            u = 2.0 * eta / 0.25
+            st = {}
+            for br in (0, 1):
+                o = O.Oracle(nx, ny, dx, 1e3, H, breaking=br, B1=0.15, B2=0.5,
+                             bc_xlo=OUT, bc_xhi=OUT, bc_ylo=PER, bc_yhi=PER)
+                o.set_state(h, h * u[None, :], 0 * h)
+                o.nonhydro_correct(1e-3)
+                st[br] = o.get_state()
+            assert np.array_equal(st[0]["h"], st[1]["h"])
+            dw = st[1]["w"] - st[0]["w"]
+            if facing > 0:
+                assert np.abs(dw).max() > 1e-6                   # R_w = 2 nu div(u) acted
+                k = np.unravel_index(np.abs(dw).argmax(), dw.shape)[1]
+                assert abs(k * dx - 3.2) < 0.5                   # ... and it acted at the front
+            else:
+                for key in st[0]:
+                    assert np.array_equal(st[0][key], st[1][key]), key
