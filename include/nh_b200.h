@@ -1,0 +1,153 @@
+/* nh_b200.h -- C ABI of libnh_b200.so: the per-time-step hot path of the hybrid finite-volume /
+ * finite-difference projection scheme of Escalante, Morales de Luna & Castro (arXiv 1706.04551,
+ * cited below as PAPER.md L<line>) for Yamazaki's depth-integrated non-hydrostatic system,
+ * hand-written CUDA for NVIDIA B200 (sm_100a), fp64, SoA.
+ *
+ * Every step of the path runs in CUDA kernels of this library; there is no CPU fallback.  No
+ * torch types appear here: plain pointers and sizes.
+ *
+ * POINTERS.  Every array pointer may be a DEVICE pointer (valid on the device of the context's
+ * stream) or a HOST pointer (pageable or pinned): copies use cudaMemcpyAsync(cudaMemcpyDefault)
+ * on the context's stream, so unified virtual addressing decides.  With pageable host memory the
+ * copy is synchronous with respect to the host.  The caller owns every buffer it passes; the
+ * library copies on create/set and copies out on get; nothing but the context is returned by
+ * pointer.  The context owns all device memory it uses (cudaMalloc at nh_create).
+ *
+ * LAYOUT.  Cell arrays: nx*ny doubles, x fastest (cell (i,j) at j*nx+i, centre ((i+1/2)dx,
+ * (j+1/2)dy)).  Node arrays: (nx+1)*(ny+1) doubles, x fastest, always; node (I,J) is the common
+ * corner of cells (I-1,J-1),(I,J-1),(I-1,J),(I,J) -- the paper's staggered point
+ * (i+1/2,j+1/2) with i=I-1, j=J-1.  In a periodic direction the
+ * last node line duplicates the first: ignored on input, filled on output.
+ *
+ * ASYNCHRONY.  nh_step / nh_hydrostatic_step / nh_nonhydro_correct / nh_set_state only enqueue
+ * work on the context's stream and return (no host synchronisation inside; dt, the solver's
+ * convergence tests and all reductions stay on the device).  nh_sync, nh_get_info, nh_get_state
+ * to a pageable host buffer, and nh_last_error synchronise.  Sticky run-time conditions (a solve
+ * that did not converge, a NaN time step) are reported by nh_sync / nh_get_info.
+ *
+ * ERRORS.  0 on success, a negative nh_status otherwise; no exceptions, no aborts, no global
+ * state.  One context may be used by one host thread at a time.
+ */
+#ifndef NH_B200_H
+#define NH_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nh_ctx nh_ctx; /* opaque */
+
+/* boundary types (the wall type is this build's extension, R9) */
+typedef enum { NH_BC_PERIODIC = 0, NH_BC_WALL = 1, NH_BC_OUTFLOW = 2 } nh_bc;
+
+typedef enum {
+  NH_OK = 0,
+  NH_EINVAL = -1,  /* invalid argument (also: h < 0 or non-finite input found by nh_sync)  */
+  NH_ENOMEM = -2,  /* host or device allocation failed                                     */
+  NH_ECUDA = -3,   /* a CUDA call failed (nh_last_error has the text)                      */
+  NH_ENOCONV = -4, /* a pressure solve hit maxit / broke down twice                        */
+  NH_ENAN = -5     /* NaN/Inf time step or right-hand side                                 */
+} nh_status;
+
+/* Parameters, passed by pointer, copied.  Fill with nh_default_params first. */
+typedef struct {
+  double g;           /* gravity, default 9.81                               */
+  double cfl;         /* CFL number in (0,1], default 0.5 (eq. (23))              */
+  double delta;       /* velocity desingularisation delta, default 1e-5 (L447-451)          */
+  double eps_dry;     /* cell is dry iff h <= eps_dry, default 1e-5 (R1)          */
+  double B1, B2;      /* breaking onset / termination coefficients, 0.15 / 0.5 (L141-143, L635) */
+  double solver_rtol; /* BiCGStab stops at ||r||_2 <= rtol ||b||_2, default 1e-12 (R14)     */
+  double gen_A, gen_h0, gen_x0, gen_Lrel; /* solitary-wave generating zone at x-lo (L417-431, R18) */
+  int breaking;       /* 1: eddy-viscosity breaking sources on (section 3, eqs (8)-(12))    */
+  int nonhydro;       /* 0: hydrostatic SWE path only (p = 0, w frozen); default 1          */
+  int time_order;     /* 1, or 2 = two-stage TVD Runge-Kutta (L406, L516, L544); default 2  */
+  int space_order;    /* 1 = eqs (16)-(19), 2 = MUSCL+minmod eqs (20)-(22); default 2       */
+  int bc_xlo, bc_xhi, bc_ylo, bc_yhi; /* nh_bc; periodic must be set on both sides of a direction */
+  int solver_maxit;   /* default 10000                                                      */
+  int gen_on;         /* 1: generating relaxation zone active                               */
+  int precision;      /* 64 (fp64).  32 is not built yet: NH_EINVAL                         */
+  int reserved;
+} nh_params;
+
+typedef struct {
+  double t;              /* simulated time                                                  */
+  double dt_last;        /* last time step used                                             */
+  double res_last;       /* last solve: true ||b-Ax||_2/||b||_2 before the polish iteration */
+  long long steps;
+  long long iters_total; /* BiCGStab iterations over all solves (polish not counted)        */
+  long long clamps;      /* number of h<0 -> 0 clamps in the predictor (R7)                 */
+  long long solves;
+  int iters_last, iters_max;
+  int flags;             /* bit0: a solve failed to converge; bit1: NaN/Inf dt or rhs;
+                            bit2: set_state saw h<0 or a non-finite value                   */
+  int reserved;
+} nh_info;
+
+void nh_default_params(nh_params* prm);
+
+/* Problem statement of the paper: a structured Cartesian mesh of nx*ny cells of size dx*dy with
+ * still-water depth H per cell (may be negative = emerged land; bed elevation z_b = -H)
+ * (PAPER.md L462-470, L528).  cuda_stream: a cudaStream_t (NULL = the default stream); all work
+ * of this context is ordered on it.  Requires nx,ny >= 4 (two-cell MUSCL halo), dx,dy > 0,
+ * finite H.  Fails with NH_ECUDA when no sm_100 device / kernel image is available. */
+int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* H,
+              const nh_params* prm, void* cuda_stream);
+void nh_destroy(nh_ctx* ctx);
+
+/* State = conserved variables (h, qx, qy) per cell (L45-59, L528) and (w, p) per staggered node
+ * (L245-247, L464-466, L535).  w, p NULL => zeros.  set validates h >= 0 and finiteness on the
+ * device (reported by nh_sync as NH_EINVAL, flag bit2). get: NULL => skip that field. */
+int nh_set_state(nh_ctx* ctx, const double* h, const double* qx, const double* qy,
+                 const double* w, const double* p);
+int nh_get_state(nh_ctx* ctx, double* h, double* qx, double* qy, double* w, double* p);
+
+/* nsteps full time steps: dt = CFL / max[(|u|+sqrt(gh))/dx + (|v|+sqrt(gh))/dy] (eq. (23),
+ * DESIGN.md R20), then per Runge-Kutta stage: hydrostatic predictor (eqs (16)-(22), (30)),
+ * breaking sources (eqs (8)-(12), (28)), pressure system assembly and BiCGStab solve (eqs
+ * (24)-(29), (36)-(43)), Chorin-Temam correction (eqs (28), (31), (41)), relaxation zone
+ * (L417-431); stages combined as U^{n+1} = (U^n + U^(2))/2 (L406, L516, L544). */
+int nh_step(nh_ctx* ctx, int nsteps);
+
+/* First part alone: predictor (S0-S5) on the current state, in place; w, p untouched.
+ * dt <= 0 => the CFL time step of the current state. */
+int nh_hydrostatic_step(nh_ctx* ctx, double dt);
+/* Second + third part alone: breaking sources, right-hand side, solve, correction (S6-S10) on
+ * the current state, in place; h unchanged.  dt > 0 required. */
+int nh_nonhydro_correct(nh_ctx* ctx, double dt);
+
+/* Wait for the stream; returns the sticky run-time status (NH_OK / NH_ENOCONV / NH_ENAN /
+ * NH_EINVAL from set_state validation / NH_ECUDA) and clears nothing. */
+int nh_sync(nh_ctx* ctx);
+int nh_get_info(nh_ctx* ctx, nh_info* out); /* synchronises */
+const char* nh_last_error(nh_ctx* ctx);
+
+/* Launch counters (host side, for bench.py's gpu_launches): number of kernels this context has
+ * launched since creation. */
+long long nh_launch_count(nh_ctx* ctx);
+
+/* Per-phase device timing for the roofline report (bench.py): when enabled, every kernel group of
+ * nh_step is bracketed by a pair of CUDA events recorded on the context's stream (no host
+ * synchronisation is added).  nh_profile_read synchronises, returns the summed milliseconds and
+ * the number of brackets per phase since the last read (arrays of NH_PROF_CATS entries, HOST
+ * pointers) and resets them.  Phases: the hydrostatic predictor (a1-a3), the assembly (a4-a5 and
+ * the rows of A), the BiCGStab solve (a6: one cooperative kernel per bracket), and the correction
+ * with the Runge-Kutta combine (a7-a8). */
+enum { NH_PROF_PREDICTOR = 0, NH_PROF_ASSEMBLY = 1, NH_PROF_SOLVER = 2, NH_PROF_CORRECT = 3,
+       NH_PROF_CATS = 4 };
+int nh_profile(nh_ctx* ctx, int enable);
+int nh_profile_read(nh_ctx* ctx, double* ms, long long* groups);
+
+/* ---- test hooks (not on the timed path); node arrays in/out use the public node layout ---- */
+int nh_compute_dt(nh_ctx* ctx, double* dt_host);          /* CFL dt of the current state; synchronises */
+int nh_apply_A(nh_ctx* ctx, const double* x_nodes, double* y_nodes); /* y = A(h,z) x, matrix-free (S8) */
+int nh_coeffs(nh_ctx* ctx, double* AC, double* AE, double* AW, double* AN, double* AS); /* rows of A */
+int nh_rhs(nh_ctx* ctx, double dt, double* b_nodes);      /* b = -B/dt of the current state (S7)   */
+int nh_constraint(nh_ctx* ctx, double* B_nodes);          /* discrete constraint B, eq. (37)       */
+/* S9 on the current state's operator: x_nodes in = start, out = solution; iters/relres are HOST
+ * pointers (may be NULL); synchronises. */
+int nh_solve(nh_ctx* ctx, const double* b_nodes, double* x_nodes, int* iters, double* relres);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,500 @@
+// nh_api.cu -- the C ABI of libnh_b200.so (include/nh_b200.h): context, state, and the step
+// driver that sequences the kernels of nh_predictor.cu / nh_pressure.cu / nh_solver.cu on the
+// context's stream.  Nothing here computes on the host: dt, the solver's convergence tests, the
+// clock and all counters stay in device memory (NhScal) until nh_get_info / nh_sync read them.
+//
+// Step order (PAPER.md L524-544 and Fig. 4, repackaged):
+//   dt = CFL / lam_max(U^n)                       (lam_max produced by the previous step's combine)
+//   for each Runge-Kutta stage:  predictor -> [breaking] -> z, rhs, rows of A -> BiCGStab
+//                                -> correction -> [relaxation zone]
+//   U^{n+1} = (U^n + U^(2)) / 2  fused with lam_max(U^{n+1})
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "nh_internal.cuh"
+
+namespace {
+
+__global__ void __launch_bounds__(256)
+k_all_finite(size_t n, const double* __restrict__ a, int* bad) {
+  bool b = false;
+  for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n;
+       k += (size_t)gridDim.x * blockDim.x) {
+    double v = a[k];
+    if (!(v == v) || isinf(v)) b = true;
+  }
+  if (__syncthreads_or(b) && threadIdx.x == 0) atomicOr(bad, 1);
+}
+
+__global__ void k_clear_flag(NhScal* sc, int mask) { sc->flags &= ~mask; }
+
+bool bc_ok(int b) { return b == NH_BC_PERIODIC || b == NH_BC_WALL || b == NH_BC_OUTFLOW; }
+
+int fail(nh_ctx* c, int code, const char* msg) {
+  if (c) snprintf(c->err, sizeof(c->err), "%s", msg);
+  return code;
+}
+
+template <typename T>
+bool dalloc(nh_ctx* c, T** p, size_t count) {
+  cudaError_t e = cudaMalloc((void**)p, count * sizeof(T));
+  if (e != cudaSuccess) {
+    *p = nullptr;
+    snprintf(c->err, sizeof(c->err), "cudaMalloc(%zu bytes): %s", count * sizeof(T),
+             cudaGetErrorString(e));
+    (void)cudaGetLastError();
+    return false;
+  }
+  e = cudaMemsetAsync(*p, 0, count * sizeof(T), c->stream);
+  return e == cudaSuccess;
+}
+
+void free_all(nh_ctx* c) {
+  double* cells[] = {c->H, c->h[0], c->h[1], c->h[2], c->qx[0], c->qx[1], c->qx[2], c->qy[0],
+                     c->qy[1], c->qy[2], c->qx1, c->qy1, c->qx2, c->qy2, c->z};
+  double* nodes[] = {c->w[0], c->w[1], c->w[2], c->w2, c->p, c->b, c->dg, c->dinv, c->cE, c->cW,
+                     c->cN, c->cS, c->ky, c->kr, c->kr0, c->kpA, c->kpB, c->kvA, c->kvB, c->kt,
+                     c->part};
+  for (double* p : cells) if (p) cudaFree(p);
+  for (double* p : nodes) if (p) cudaFree(p);
+  if (c->flag_c) cudaFree(c->flag_c);
+  if (c->flag_n) cudaFree(c->flag_n);
+  if (c->sc) cudaFree(c->sc);
+  if (c->sc_host) cudaFreeHost(c->sc_host);
+  for (int k = 0; k < NH_PROF_CATS; ++k)
+    for (auto& ev : c->prof_ev[k]) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
+}
+
+// copy in/out with cudaMemcpyDefault: the pointer may be host or device (UVA decides)
+int copy_async(nh_ctx* c, void* dst, const void* src, size_t bytes) {
+  cudaError_t e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDefault, c->stream);
+  if (e != cudaSuccess) {
+    snprintf(c->err, sizeof(c->err), "cudaMemcpyAsync: %s", cudaGetErrorString(e));
+    (void)cudaGetLastError();
+    c->host_status = NH_ECUDA;
+    return NH_ECUDA;
+  }
+  return NH_OK;
+}
+
+int check_launch(nh_ctx* c) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) {
+    snprintf(c->err, sizeof(c->err), "kernel launch: %s", cudaGetErrorString(e));
+    c->host_status = NH_ECUDA;
+    return NH_ECUDA;
+  }
+  return c->host_status;
+}
+
+int sticky_status(nh_ctx* c, int flags) {
+  if (c->host_status != NH_OK) return c->host_status;
+  if (flags & NH_FLAG_NAN) return fail(c, NH_ENAN, "NaN/Inf time step or right-hand side");
+  if (flags & NH_FLAG_NOCONV) return fail(c, NH_ENOCONV, "step: pressure solve did not converge");
+  return NH_OK;
+}
+
+int read_scalars(nh_ctx* c) {
+  cudaError_t e = cudaMemcpyAsync(c->sc_host, c->sc, sizeof(NhScal), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) {
+    snprintf(c->err, sizeof(c->err), "synchronise: %s", cudaGetErrorString(e));
+    c->host_status = NH_ECUDA;
+    return NH_ECUDA;
+  }
+  return NH_OK;
+}
+
+// other two slots, given the current one
+inline void other_slots(int cur, int& s1, int& s2) { s1 = (cur + 1) % 3; s2 = (cur + 2) % 3; }
+
+struct ProfScope {  // CUDA-event bracket of one kernel group on the context's stream
+  nh_ctx* c; int cat; cudaEvent_t e0, e1; bool on;
+  ProfScope(nh_ctx* c_, int cat_) : c(c_), cat(cat_), on(c_->prof_on) {
+    if (!on) return;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    cudaEventRecord(e0, c->stream);
+  }
+  ~ProfScope() {
+    if (!on) return;
+    cudaEventRecord(e1, c->stream);
+    c->prof_ev[cat].push_back({e0, e1});
+  }
+};
+
+// S6-S10 on U* = (h1, qx1, qy1) with w_in -> (qx_out, qy_out, w_out); p~ in c->p (warm start).
+void nonhydro_part(nh_ctx* c, const double* h1, const double* qx1, const double* qy1,
+                   const double* w_in, double* qx_out, double* qy_out, double* w_out) {
+  const double *qxs = qx1, *qys = qy1, *ws = w_in;
+  {
+    ProfScope ps(c, NH_PROF_ASSEMBLY);
+    if (c->prm.breaking) {
+      nh_launch_breaking(c, h1, qx1, qy1, w_in, c->qx2, c->qy2, c->w2);
+      qxs = c->qx2; qys = c->qy2; ws = c->w2;
+    }
+    nh_launch_compute_z(c, h1, c->z);
+    nh_launch_rhs(c, h1, qxs, qys, c->z, ws, c->b, 0);
+    nh_launch_coeffs(c, h1, c->z);
+    nh_launch_scale_coeffs(c);
+  }
+  {
+    ProfScope ps(c, NH_PROF_SOLVER);
+    nh_launch_solve(c, c->b, c->p, 1);
+  }
+  {
+    ProfScope ps(c, NH_PROF_CORRECT);
+    nh_launch_correct(c, h1, c->z, qxs, qys, ws, c->p, qx_out, qy_out, w_out);
+  }
+}
+
+// w changes within a stage only through the correction (nonhydro) or the relaxation zone
+inline bool w_moves(const nh_ctx* c) { return c->prm.nonhydro || c->prm.gen_on; }
+
+// one stage Phi_dt: cell slot `in` -> `out`, node slot `inw` -> `outw` (== inw when w does not
+// move); stage_idx selects the relaxation clock (end time of the stage).
+void stage(nh_ctx* c, int in, int inw, int out, int outw, int stage_idx) {
+  if (c->prm.nonhydro) {
+    {
+      ProfScope ps(c, NH_PROF_PREDICTOR);
+      nh_launch_predictor(c, c->h[in], c->qx[in], c->qy[in], c->h[out], c->qx1, c->qy1);
+    }
+    nonhydro_part(c, c->h[out], c->qx1, c->qy1, c->w[inw], c->qx[out], c->qy[out], c->w[outw]);
+  } else {
+    ProfScope ps(c, NH_PROF_PREDICTOR);
+    nh_launch_predictor(c, c->h[in], c->qx[in], c->qy[in], c->h[out], c->qx[out], c->qy[out]);
+    if (outw != inw) copy_async(c, c->w[outw], c->w[inw], c->nn * sizeof(double));
+  }
+  if (c->prm.gen_on)
+    nh_launch_relax(c, c->h[out], c->qx[out], c->qy[out], c->w[outw], c->p, stage_idx);
+}
+
+void ensure_lambda(nh_ctx* c) {
+  if (!c->lam_valid) nh_launch_lambda(c, c->h[c->cur], c->qx[c->cur], c->qy[c->cur]);
+}
+
+}  // namespace
+
+extern "C" {
+
+void nh_default_params(nh_params* prm) {
+  if (!prm) return;
+  memset(prm, 0, sizeof(*prm));
+  prm->g = 9.81; prm->cfl = 0.5; prm->delta = 1e-5; prm->eps_dry = 1e-5;
+  prm->B1 = 0.15; prm->B2 = 0.5; prm->solver_rtol = 1e-12;
+  prm->breaking = 0; prm->nonhydro = 1; prm->time_order = 2; prm->space_order = 2;
+  prm->bc_xlo = prm->bc_xhi = prm->bc_ylo = prm->bc_yhi = NH_BC_OUTFLOW;
+  prm->solver_maxit = 10000; prm->gen_on = 0; prm->precision = 64;
+}
+
+int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* H,
+              const nh_params* prm, void* cuda_stream) {
+  if (!out || !H || !prm) return NH_EINVAL;
+  *out = nullptr;
+  if (nx < 4 || ny < 4 || !(dx > 0.0) || !(dy > 0.0)) return NH_EINVAL;
+  if (!(prm->cfl > 0.0 && prm->cfl <= 1.0) || !(prm->g > 0.0) || !(prm->delta > 0.0)) return NH_EINVAL;
+  if (!(prm->eps_dry >= 0.0) || !(prm->solver_rtol > 0.0) || prm->solver_maxit < 1) return NH_EINVAL;
+  if (!bc_ok(prm->bc_xlo) || !bc_ok(prm->bc_xhi) || !bc_ok(prm->bc_ylo) || !bc_ok(prm->bc_yhi)) return NH_EINVAL;
+  if ((prm->bc_xlo == NH_BC_PERIODIC) != (prm->bc_xhi == NH_BC_PERIODIC)) return NH_EINVAL;
+  if ((prm->bc_ylo == NH_BC_PERIODIC) != (prm->bc_yhi == NH_BC_PERIODIC)) return NH_EINVAL;
+  if (prm->time_order != 1 && prm->time_order != 2) return NH_EINVAL;
+  if (prm->space_order != 1 && prm->space_order != 2) return NH_EINVAL;
+  if (prm->precision != 64) return NH_EINVAL;
+  if (prm->breaking && !(prm->B1 > 0.0 && prm->B2 > 0.0)) return NH_EINVAL;
+  if (prm->gen_on && !(prm->gen_A > 0.0 && prm->gen_h0 > 0.0 && prm->gen_Lrel > 0.0)) return NH_EINVAL;
+
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return NH_ECUDA; }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { (void)cudaGetLastError(); return NH_ECUDA; }
+  if (prop.major != 10) return NH_ECUDA;  // the library carries sm_100a code only
+
+  nh_ctx* c = new (std::nothrow) nh_ctx();
+  if (!c) return NH_ENOMEM;
+  c->g.nx = nx; c->g.ny = ny; c->g.dx = dx; c->g.dy = dy;
+  c->g.bxlo = prm->bc_xlo; c->g.bxhi = prm->bc_xhi; c->g.bylo = prm->bc_ylo; c->g.byhi = prm->bc_yhi;
+  c->g.nnx = (prm->bc_xlo == NH_BC_PERIODIC) ? nx : nx + 1;
+  c->g.nny = (prm->bc_ylo == NH_BC_PERIODIC) ? ny : ny + 1;
+  c->g.np = nx + 1;
+  c->prm = *prm;
+  c->stream = (cudaStream_t)cuda_stream;
+  c->device = dev;
+  c->sm_count = prop.multiProcessorCount;
+  c->nc = (size_t)nx * ny;
+  c->nn = (size_t)(nx + 1) * (ny + 1);
+  c->cur = 0; c->curw = 0;
+  c->lam_valid = false;
+  c->host_status = NH_OK;
+
+  bool ok = true;
+  double** cells[] = {&c->H, &c->h[0], &c->h[1], &c->h[2], &c->qx[0], &c->qx[1], &c->qx[2],
+                      &c->qy[0], &c->qy[1], &c->qy[2], &c->qx1, &c->qy1, &c->z};
+  double** nodes[] = {&c->w[0], &c->w[1], &c->w[2], &c->p, &c->b, &c->dg, &c->dinv, &c->cE, &c->cW,
+                      &c->cN, &c->cS, &c->ky, &c->kr, &c->kr0, &c->kpA, &c->kpB, &c->kvA, &c->kvB,
+                      &c->kt, &c->w2};
+  for (double** p : cells) ok = ok && dalloc(c, p, c->nc);
+  for (double** p : nodes) ok = ok && dalloc(c, p, c->nn);
+  if (prm->breaking) {
+    ok = ok && dalloc(c, &c->qx2, c->nc) && dalloc(c, &c->qy2, c->nc);
+    ok = ok && dalloc(c, &c->flag_c, c->nc) && dalloc(c, &c->flag_n, c->nn);
+  }
+  ok = ok && dalloc(c, &c->sc, 1);
+  if (ok && cudaMallocHost((void**)&c->sc_host, sizeof(NhScal)) != cudaSuccess) ok = false;
+  if (ok && nh_solver_setup(c) != NH_OK) ok = false;
+  if (!ok) { (void)cudaGetLastError(); free_all(c); delete c; return NH_ENOMEM; }
+
+  // bathymetry: copy, then validate finiteness on the device (create may synchronise)
+  int st = copy_async(c, c->H, H, c->nc * sizeof(double));
+  int* bad = (int*)&c->sc->pad;
+  if (st == NH_OK) {
+    size_t nb = (c->nc + 255) / 256, cap = (size_t)c->sm_count * 16;
+    k_all_finite<<<(int)(nb < cap ? nb : cap), 256, 0, c->stream>>>(c->nc, c->H, bad);
+    c->launches++;
+    st = check_launch(c);
+  }
+  if (st == NH_OK) st = read_scalars(c);
+  if (st == NH_OK && c->sc_host->pad != 0) st = NH_EINVAL;
+  if (st != NH_OK) { free_all(c); delete c; return st; }
+  cudaMemsetAsync(c->sc, 0, sizeof(NhScal), c->stream);
+  *out = c;
+  return NH_OK;
+}
+
+void nh_destroy(nh_ctx* c) {
+  if (!c) return;
+  cudaStreamSynchronize(c->stream);
+  free_all(c);
+  delete c;
+}
+
+int nh_set_state(nh_ctx* c, const double* h, const double* qx, const double* qy, const double* w,
+                 const double* p) {
+  if (!c || !h || !qx || !qy) return NH_EINVAL;
+  int s1, s2; other_slots(c->cur, s1, s2);
+  size_t cb = c->nc * sizeof(double), nb = c->nn * sizeof(double);
+  // stage into a free slot, validate there, then make it current (an invalid state changes nothing)
+  if (copy_async(c, c->h[s1], h, cb) || copy_async(c, c->qx[s1], qx, cb) ||
+      copy_async(c, c->qy[s1], qy, cb))
+    return NH_ECUDA;
+  k_clear_flag<<<1, 1, 0, c->stream>>>(c->sc, NH_FLAG_BADSTATE);
+  c->launches++;
+  nh_launch_validate(c, c->h[s1], c->qx[s1], c->qy[s1]);
+  if (check_launch(c) != NH_OK) return NH_ECUDA;
+  if (read_scalars(c) != NH_OK) return NH_ECUDA;
+  if (c->sc_host->flags & NH_FLAG_BADSTATE)
+    return fail(c, NH_EINVAL, "set_state: h<0 or non-finite input");
+  c->cur = s1;
+  if (w) { if (copy_async(c, c->w[c->curw], w, nb)) return NH_ECUDA; }
+  else cudaMemsetAsync(c->w[c->curw], 0, nb, c->stream);
+  if (p) { if (copy_async(c, c->p, p, nb)) return NH_ECUDA; }
+  else cudaMemsetAsync(c->p, 0, nb, c->stream);
+  c->lam_valid = false;
+  return NH_OK;
+}
+
+// node array out in the public layout (periodic duplicate lines filled), via scratch
+static int node_out(nh_ctx* c, const double* src, double* dst_user, double* scratch) {
+  nh_launch_nodes_out(c, src, scratch);
+  if (check_launch(c) != NH_OK) return NH_ECUDA;
+  return copy_async(c, dst_user, scratch, c->nn * sizeof(double));
+}
+
+int nh_get_state(nh_ctx* c, double* h, double* qx, double* qy, double* w, double* p) {
+  if (!c) return NH_EINVAL;
+  size_t cb = c->nc * sizeof(double);
+  if (h && copy_async(c, h, c->h[c->cur], cb)) return NH_ECUDA;
+  if (qx && copy_async(c, qx, c->qx[c->cur], cb)) return NH_ECUDA;
+  if (qy && copy_async(c, qy, c->qy[c->cur], cb)) return NH_ECUDA;
+  // kt / kr are solver scratch, free between solves
+  if (w && node_out(c, c->w[c->curw], w, c->kt)) return NH_ECUDA;
+  if (p && node_out(c, c->p, p, c->kr)) return NH_ECUDA;
+  cudaError_t e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) { c->host_status = NH_ECUDA; return fail(c, NH_ECUDA, cudaGetErrorString(e)); }
+  return NH_OK;
+}
+
+int nh_step(nh_ctx* c, int nsteps) {
+  if (!c || nsteps < 0) return NH_EINVAL;
+  if (c->host_status != NH_OK) return c->host_status;
+  for (int s = 0; s < nsteps; ++s) {
+    ensure_lambda(c);
+    nh_launch_set_dt(c, 0.0);
+    c->lam_valid = false;
+    int s1, s2, w1, w2;
+    other_slots(c->cur, s1, s2);
+    other_slots(c->curw, w1, w2);
+    if (!w_moves(c)) w1 = w2 = c->curw;
+    if (c->prm.time_order == 1) {
+      stage(c, c->cur, c->curw, s1, w1, 0);
+      c->cur = s1; c->curw = w1;
+    } else {
+      stage(c, c->cur, c->curw, s1, w1, 0);
+      stage(c, s1, w1, s2, w2, 1);
+      ProfScope ps(c, NH_PROF_CORRECT);
+      nh_launch_combine(c, c->h[c->cur], c->qx[c->cur], c->qy[c->cur], c->w[c->curw], c->h[s2],
+                        c->qx[s2], c->qy[s2], c->w[w2]);
+      c->lam_valid = true;
+    }
+    nh_launch_end_step(c, 1);
+  }
+  return check_launch(c);
+}
+
+int nh_hydrostatic_step(nh_ctx* c, double dt) {
+  if (!c) return NH_EINVAL;
+  if (c->host_status != NH_OK) return c->host_status;
+  if (!(dt > 0.0)) { ensure_lambda(c); nh_launch_set_dt(c, 0.0); }
+  else nh_launch_set_dt(c, dt);
+  c->lam_valid = false;
+  int s1, s2; other_slots(c->cur, s1, s2);
+  nh_launch_predictor(c, c->h[c->cur], c->qx[c->cur], c->qy[c->cur], c->h[s1], c->qx[s1], c->qy[s1]);
+  c->cur = s1;
+  nh_launch_end_step(c, 0);
+  return check_launch(c);
+}
+
+int nh_nonhydro_correct(nh_ctx* c, double dt) {
+  if (!c || !(dt > 0.0)) return NH_EINVAL;
+  if (c->host_status != NH_OK) return c->host_status;
+  nh_launch_set_dt(c, dt);
+  c->lam_valid = false;
+  int s1, s2, w1, w2;
+  other_slots(c->cur, s1, s2);
+  other_slots(c->curw, w1, w2);
+  // U* := current state; h is not changed by S6-S10
+  nonhydro_part(c, c->h[c->cur], c->qx[c->cur], c->qy[c->cur], c->w[c->curw], c->qx[s1], c->qy[s1],
+                c->w[w1]);
+  if (copy_async(c, c->h[s1], c->h[c->cur], c->nc * sizeof(double))) return NH_ECUDA;
+  c->cur = s1; c->curw = w1;
+  nh_launch_end_step(c, 0);
+  return check_launch(c);
+}
+
+int nh_sync(nh_ctx* c) {
+  if (!c) return NH_EINVAL;
+  if (read_scalars(c) != NH_OK) return NH_ECUDA;
+  return sticky_status(c, c->sc_host->flags);
+}
+
+int nh_get_info(nh_ctx* c, nh_info* out) {
+  if (!c || !out) return NH_EINVAL;
+  if (read_scalars(c) != NH_OK) return NH_ECUDA;
+  const NhScal& s = *c->sc_host;
+  memset(out, 0, sizeof(*out));
+  out->t = s.t; out->dt_last = s.dt_last; out->res_last = s.res_last;
+  out->steps = s.steps; out->iters_total = s.iters_total; out->clamps = s.clamps;
+  out->solves = s.solves; out->iters_last = s.iters_last; out->iters_max = s.iters_max;
+  out->flags = s.flags;
+  return NH_OK;
+}
+
+const char* nh_last_error(nh_ctx* c) { return c ? c->err : "null context"; }
+
+long long nh_launch_count(nh_ctx* c) { return c ? c->launches : 0; }
+
+// ---- per-phase device timing (bench.py's roofline: CUDA events on the context's stream) ----
+int nh_profile(nh_ctx* c, int enable) {
+  if (!c) return NH_EINVAL;
+  cudaStreamSynchronize(c->stream);
+  for (int k = 0; k < NH_PROF_CATS; ++k) {
+    for (auto& ev : c->prof_ev[k]) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
+    c->prof_ev[k].clear();
+  }
+  c->prof_on = enable != 0;
+  return NH_OK;
+}
+
+int nh_profile_read(nh_ctx* c, double* ms, long long* groups) {
+  if (!c || !ms || !groups) return NH_EINVAL;
+  cudaError_t e = cudaStreamSynchronize(c->stream);
+  if (e != cudaSuccess) { c->host_status = NH_ECUDA; return fail(c, NH_ECUDA, cudaGetErrorString(e)); }
+  for (int k = 0; k < NH_PROF_CATS; ++k) {
+    double tot = 0.0;
+    for (auto& ev : c->prof_ev[k]) {
+      float t = 0.f;
+      if (cudaEventElapsedTime(&t, ev.first, ev.second) == cudaSuccess) tot += t;
+      cudaEventDestroy(ev.first); cudaEventDestroy(ev.second);
+    }
+    ms[k] = tot;
+    groups[k] = (long long)c->prof_ev[k].size();
+    c->prof_ev[k].clear();
+  }
+  return NH_OK;
+}
+
+// ---- test hooks (not on the timed path) ----------------------------------------------------
+int nh_compute_dt(nh_ctx* c, double* dt_host) {
+  if (!c || !dt_host) return NH_EINVAL;
+  ensure_lambda(c);
+  nh_launch_set_dt(c, 0.0);
+  c->lam_valid = false;
+  if (check_launch(c) != NH_OK) return NH_ECUDA;
+  if (read_scalars(c) != NH_OK) return NH_ECUDA;
+  *dt_host = c->sc_host->dt;
+  return NH_OK;
+}
+
+int nh_apply_A(nh_ctx* c, const double* x_nodes, double* y_nodes) {
+  if (!c || !x_nodes || !y_nodes) return NH_EINVAL;
+  if (copy_async(c, c->kpA, x_nodes, c->nn * sizeof(double))) return NH_ECUDA;
+  nh_launch_compute_z(c, c->h[c->cur], c->z);
+  nh_launch_apply_A(c, c->h[c->cur], c->z, c->kpA, c->kpB);
+  if (node_out(c, c->kpB, y_nodes, c->kvA)) return NH_ECUDA;
+  cudaStreamSynchronize(c->stream);
+  return check_launch(c);
+}
+
+int nh_coeffs(nh_ctx* c, double* AC, double* AE, double* AW, double* AN, double* AS) {
+  if (!c || !AC || !AE || !AW || !AN || !AS) return NH_EINVAL;
+  nh_launch_compute_z(c, c->h[c->cur], c->z);
+  nh_launch_coeffs(c, c->h[c->cur], c->z);  // raw (unscaled) rows
+  const double* src[5] = {c->dg, c->cE, c->cW, c->cN, c->cS};
+  double* dst[5] = {AC, AE, AW, AN, AS};
+  for (int k = 0; k < 5; ++k)
+    if (node_out(c, src[k], dst[k], c->kvA)) return NH_ECUDA;
+  cudaStreamSynchronize(c->stream);
+  return check_launch(c);
+}
+
+static int rhs_hook(nh_ctx* c, double dt, double* out, int constraint_only) {
+  if (!constraint_only) { nh_launch_set_dt(c, dt); c->lam_valid = false; }
+  nh_launch_compute_z(c, c->h[c->cur], c->z);
+  nh_launch_rhs(c, c->h[c->cur], c->qx[c->cur], c->qy[c->cur], c->z, c->w[c->curw], c->b,
+                constraint_only);
+  if (node_out(c, c->b, out, c->kvA)) return NH_ECUDA;
+  cudaStreamSynchronize(c->stream);
+  return check_launch(c);
+}
+int nh_rhs(nh_ctx* c, double dt, double* b_nodes) {
+  if (!c || !b_nodes || !(dt > 0.0)) return NH_EINVAL;
+  return rhs_hook(c, dt, b_nodes, 0);
+}
+int nh_constraint(nh_ctx* c, double* B_nodes) {
+  if (!c || !B_nodes) return NH_EINVAL;
+  return rhs_hook(c, 1.0, B_nodes, 1);
+}
+
+int nh_solve(nh_ctx* c, const double* b_nodes, double* x_nodes, int* iters, double* relres) {
+  if (!c || !b_nodes || !x_nodes) return NH_EINVAL;
+  size_t nb = c->nn * sizeof(double);
+  if (copy_async(c, c->b, b_nodes, nb) || copy_async(c, c->w2, x_nodes, nb)) return NH_ECUDA;
+  nh_launch_compute_z(c, c->h[c->cur], c->z);
+  nh_launch_coeffs(c, c->h[c->cur], c->z);
+  nh_launch_scale_coeffs(c);
+  nh_launch_solve(c, c->b, c->w2, 0);
+  if (node_out(c, c->w2, x_nodes, c->kvA)) return NH_ECUDA;
+  if (check_launch(c) != NH_OK) return NH_ECUDA;
+  if (read_scalars(c) != NH_OK) return NH_ECUDA;
+  if (iters) *iters = c->sc_host->iters_last;
+  if (relres) *relres = c->sc_host->res_last;
+  int fl = c->sc_host->flags;
+  // the hook reports its own solve; clear the sticky bits it may have set
+  k_clear_flag<<<1, 1, 0, c->stream>>>(c->sc, NH_FLAG_NOCONV | NH_FLAG_NAN);
+  c->launches++;
+  if (fl & NH_FLAG_NAN) return NH_ENAN;
+  if (fl & NH_FLAG_NOCONV) return NH_ENOCONV;
+  return NH_OK;
+}
+
+}  // extern "C"

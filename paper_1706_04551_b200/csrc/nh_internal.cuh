@@ -1,0 +1,172 @@
+// nh_internal.cuh -- shared declarations of the CUDA path (libnh_b200.so).  Not part of the ABI.
+//
+// Steps S0..S11 and readings R1..R23 are those of DESIGN.md (restating SURVEY.md 8(c));
+// "L<n>" are PAPER.md line numbers (arXiv 1706.04551).
+//
+// Arithmetic contract: fp64, compiled with -fmad=false so that every formula is evaluated in
+// source order with IEEE-754 round-to-nearest operations (CUDA's fp64 div and sqrt are correctly
+// rounded).  The predictor, the breaking sources, the right-hand side, the coefficients and the
+// correction therefore take every discrete decision (minmod branch, wet/dry test, emerging-bottom
+// clip, breaking flag, clamp) on the same values a plain CPU evaluation of the paper's formulas
+// sees; only the Krylov solver's dot products are summed in a different (tree) order.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <utility>
+#include <vector>
+
+#include "../../include/nh_b200.h"
+
+struct NhGrid {
+  int nx, ny;    // cells
+  int nnx, nny;  // distinct node lines: n in a periodic direction, n+1 otherwise
+  int np;        // node pitch = nx+1 (public node layout, kept internally)
+  int bxlo, bxhi, bylo, byhi;
+  double dx, dy;
+};
+
+// Device-resident scalars: the time step, the clock and the counters never visit the host
+// inside nh_step.
+struct NhScal {
+  double dt;        // time step of the step in flight
+  double t;         // simulated time
+  double dt_last;
+  double res_last;
+  unsigned long long lam_bits;  // max over cells of the CFL rate, as the bits of a non-negative double
+  long long steps, iters_total, clamps, solves;
+  int iters_last, iters_max, flags, pad;
+};
+
+enum { NH_FLAG_NOCONV = 1, NH_FLAG_NAN = 2, NH_FLAG_BADSTATE = 4 };
+
+// ---- S1: ghost access by index maps (R9) ------------------------------------------------
+// cells: periodic wraps; wall / outflow mirror (-1->0, -2->1, n->n-1, n+1->n-2); sgn = -1 only
+// in a wall ghost (applied by the caller to the normal discharge / velocity).
+__device__ __forceinline__ int nh_map_cell(int i, int n, int bclo, int bchi, double& sgn) {
+  sgn = 1.0;
+  if (i < 0) {
+    if (bclo == NH_BC_PERIODIC) return i + n;
+    if (bclo == NH_BC_WALL) sgn = -1.0;
+    return -1 - i;
+  }
+  if (i >= n) {
+    if (bchi == NH_BC_PERIODIC) return i - n;
+    if (bchi == NH_BC_WALL) sgn = -1.0;
+    return 2 * n - 1 - i;
+  }
+  return i;
+}
+__device__ __forceinline__ int nh_map_cell_even(int i, int n, int bclo, int bchi) {
+  if (i < 0) return (bclo == NH_BC_PERIODIC) ? i + n : -1 - i;
+  if (i >= n) return (bchi == NH_BC_PERIODIC) ? i - n : 2 * n - 1 - i;
+  return i;
+}
+// nodes: periodic: node n == node 0 (n distinct lines, n = number of cells); mirror: -1 -> 1,
+// n+1 -> n-1 (R10).  Valid for -n <= I <= 2n.
+__device__ __forceinline__ int nh_map_node(int I, int n, int bclo) {
+  if (bclo == NH_BC_PERIODIC) {
+    if (I < 0) return I + n;
+    if (I >= n) return I - n;
+    return I;
+  }
+  if (I < 0) return -I;
+  if (I > n) return 2 * n - I;
+  return I;
+}
+
+// S0: desingularised velocity u = sqrt(2) h q / sqrt(h^4 + max(h^4, delta^4))  (L447-451)
+#define NH_SQRT2 1.4142135623730951
+__device__ __forceinline__ double nh_dsg(double h, double q, double delta) {
+  double h2 = h * h, h4 = h2 * h2;
+  double d2 = delta * delta, d4 = d2 * d2;
+  double den = sqrt(h4 + fmax(h4, d4));
+  return (NH_SQRT2 * h * q) / den;
+}
+// R16: dinv(h) = sqrt(2) h / sqrt(h^4 + max(h^4, delta^4))  (= 1/h for h >= delta)
+__device__ __forceinline__ double nh_dinv_h(double h, double delta) {
+  double h2 = h * h, h4 = h2 * h2;
+  double d2 = delta * delta, d4 = d2 * d2;
+  return (NH_SQRT2 * h) / sqrt(h4 + fmax(h4, d4));
+}
+// S2: minmod(a,b) = 0 if ab <= 0 else sign(a) min(|a|,|b|)  (L335)
+__device__ __forceinline__ double nh_minmod(double a, double b) {
+  if (a * b <= 0.0) return 0.0;
+  return (a > 0.0) ? fmin(a, b) : fmax(a, b);
+}
+
+// ---- context ------------------------------------------------------------------------------
+struct nh_ctx {
+  NhGrid g;
+  nh_params prm;
+  cudaStream_t stream;
+  int device;
+  int sm_count;
+  long long launches;
+  char err[512];
+  int host_status;  // sticky host-side error (NH_ECUDA)
+  bool lam_valid;   // sc->lam_bits holds the CFL rate of the current state
+
+  size_t nc, nn;  // cells, nodes (public node layout)
+  // cells
+  double* H;
+  double *h[3], *qx[3], *qy[3];  // three state slots (rotating): current, stage 1, stage 2
+  double *qx1, *qy1;             // predictor output q*
+  double *qx2, *qy2;             // q** (breaking on)
+  double* z;                     // z = 2 eta - h of U*
+  unsigned char *flag_c, *flag_n;
+  // nodes
+  double* w[3];
+  double* w2;  // w** (breaking on)
+  double* p;   // pressure multiplier p~ (warm start of the next solve)
+  double* b;   // right-hand side
+  double *dg, *dinv, *cE, *cW, *cN, *cS;  // diag(A), its inverse, column-scaled off-diagonals
+  double *ky, *kr, *kr0, *kpA, *kpB, *kvA, *kvB, *kt;  // BiCGStab vectors
+  double* part;  // per-CTA partial sums of the solver
+  int solver_grid, solver_occ;
+  NhScal* sc;       // device scalars
+  NhScal* sc_host;  // pinned mirror
+  int cur;          // index of the cell slot (h, qx, qy) holding the current state
+  int curw;         // index of the node slot (w) holding the current state
+  // per-phase CUDA-event brackets (nh_profile): predictor / assembly / solver / correction
+  bool prof_on;
+  std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev[NH_PROF_CATS];
+};
+
+// ---- kernel launchers (each enqueues on c->stream and bumps c->launches) --------------------
+// nh_predictor.cu
+void nh_launch_lambda(nh_ctx* c, const double* h, const double* qx, const double* qy);
+void nh_launch_set_dt(nh_ctx* c, double dt_fixed /* <=0: CFL from lam */);
+void nh_launch_end_step(nh_ctx* c, int advance_time);
+void nh_launch_predictor(nh_ctx* c, const double* h, const double* qx, const double* qy,
+                         double* h1, double* qx1, double* qy1);
+void nh_launch_combine(nh_ctx* c, double* h0, double* qx0, double* qy0, double* w0,
+                       const double* h2, const double* qx2, const double* qy2, const double* w2);
+void nh_launch_validate(nh_ctx* c, const double* h, const double* qx, const double* qy);
+// nh_pressure.cu
+void nh_launch_compute_z(nh_ctx* c, const double* h, double* z);
+void nh_launch_breaking(nh_ctx* c, const double* h, const double* qx1, const double* qy1,
+                        const double* w_in, double* qx2, double* qy2, double* w2);
+void nh_launch_rhs(nh_ctx* c, const double* h, const double* qx, const double* qy, const double* z,
+                   const double* w, double* b, int constraint_only);
+void nh_launch_coeffs(nh_ctx* c, const double* h, const double* z);  // -> dg, dinv, raw cE..cS
+void nh_launch_scale_coeffs(nh_ctx* c);                              // cX *= dinv(neighbour)
+void nh_launch_apply_A(nh_ctx* c, const double* h, const double* z, const double* x, double* y);
+void nh_launch_correct(nh_ctx* c, const double* h, const double* z, const double* qx2,
+                       const double* qy2, const double* w2, const double* p, double* qx_out,
+                       double* qy_out, double* w_out);
+void nh_launch_relax(nh_ctx* c, double* h, double* qx, double* qy, double* w, double* p, int stage);
+void nh_launch_nodes_out(nh_ctx* c, const double* src, double* dst);
+// nh_solver.cu
+int nh_solver_setup(nh_ctx* c);  // occupancy -> cooperative grid, partial buffer
+void nh_launch_solve(nh_ctx* c, const double* b, double* x, int count_stats);
+
+#define NH_CUDA_OK(c, call)                                                                   \
+  do {                                                                                        \
+    cudaError_t e_ = (call);                                                                  \
+    if (e_ != cudaSuccess) {                                                                  \
+      snprintf((c)->err, sizeof((c)->err), "%s:%d: %s: %s", __FILE__, __LINE__, #call,        \
+               cudaGetErrorString(e_));                                                       \
+      (c)->host_status = NH_ECUDA;                                                            \
+    }                                                                                         \
+  } while (0)
