@@ -47,21 +47,24 @@ bool dalloc(nh_ctx* c, T** p, size_t count) {
     (void)cudaGetLastError();
     return false;
   }
+  c->raw.push_back((void*)*p);
   e = cudaMemsetAsync(*p, 0, count * sizeof(T), c->stream);
   return e == cudaSuccess;
 }
 
+// internal node plane (ghost ring, nh_internal.cuh): the handed-out pointer addresses node (0,0)
+inline size_t node_origin(const nh_ctx* c) { return (size_t)NH_ROW_PAD * c->g.np + 2; }
+bool nalloc(nh_ctx* c, double** p) {
+  double* base = nullptr;
+  if (!dalloc(c, &base, c->nni)) { *p = nullptr; return false; }
+  *p = base + node_origin(c);
+  return true;
+}
+
 void free_all(nh_ctx* c) {
-  double* cells[] = {c->H, c->h[0], c->h[1], c->h[2], c->qx[0], c->qx[1], c->qx[2], c->qy[0],
-                     c->qy[1], c->qy[2], c->qx1, c->qy1, c->qx2, c->qy2, c->z};
-  double* nodes[] = {c->w[0], c->w[1], c->w[2], c->w2, c->p, c->b, c->dg, c->dinv, c->cE, c->cW,
-                     c->cN, c->cS, c->ky, c->kr, c->kr0, c->kpA, c->kpB, c->kvA, c->kvB, c->kt,
-                     c->part};
-  for (double* p : cells) if (p) cudaFree(p);
-  for (double* p : nodes) if (p) cudaFree(p);
-  if (c->flag_c) cudaFree(c->flag_c);
-  if (c->flag_n) cudaFree(c->flag_n);
-  if (c->sc) cudaFree(c->sc);
+  for (void* p : c->raw) if (p) cudaFree(p);
+  c->raw.clear();
+  if (c->part) cudaFree(c->part);
   if (c->sc_host) cudaFreeHost(c->sc_host);
   for (int k = 0; k < NH_PROF_CATS; ++k)
     for (auto& ev : c->prof_ev[k]) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
@@ -72,6 +75,26 @@ int copy_async(nh_ctx* c, void* dst, const void* src, size_t bytes) {
   cudaError_t e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDefault, c->stream);
   if (e != cudaSuccess) {
     snprintf(c->err, sizeof(c->err), "cudaMemcpyAsync: %s", cudaGetErrorString(e));
+    (void)cudaGetLastError();
+    c->host_status = NH_ECUDA;
+    return NH_ECUDA;
+  }
+  return NH_OK;
+}
+
+// public node array (dense (nx+1) x (ny+1), host or device) -> internal plane: the distinct lines
+// only (a periodic duplicate line is ignored on input); NULL -> zeros
+int node_in(nh_ctx* c, double* dst, const double* src_user) {
+  cudaError_t e;
+  if (!src_user) {
+    e = cudaMemsetAsync(dst - node_origin(c), 0, c->nni * sizeof(double), c->stream);
+  } else {
+    e = cudaMemcpy2DAsync(dst, (size_t)c->g.np * sizeof(double), src_user,
+                          (size_t)(c->g.nx + 1) * sizeof(double), (size_t)c->g.nnx * sizeof(double),
+                          (size_t)c->g.nny, cudaMemcpyDefault, c->stream);
+  }
+  if (e != cudaSuccess) {
+    snprintf(c->err, sizeof(c->err), "node copy in: %s", cudaGetErrorString(e));
     (void)cudaGetLastError();
     c->host_status = NH_ECUDA;
     return NH_ECUDA;
@@ -164,7 +187,8 @@ void stage(nh_ctx* c, int in, int inw, int out, int outw, int stage_idx) {
   } else {
     ProfScope ps(c, NH_PROF_PREDICTOR);
     nh_launch_predictor(c, c->h[in], c->qx[in], c->qy[in], c->h[out], c->qx[out], c->qy[out]);
-    if (outw != inw) copy_async(c, c->w[outw], c->w[inw], c->nn * sizeof(double));
+    if (outw != inw)
+      copy_async(c, c->w[outw] - node_origin(c), c->w[inw] - node_origin(c), c->nni * sizeof(double));
   }
   if (c->prm.gen_on)
     nh_launch_relax(c, c->h[out], c->qx[out], c->qy[out], c->w[outw], c->p, stage_idx);
@@ -216,13 +240,14 @@ int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* 
   c->g.bxlo = prm->bc_xlo; c->g.bxhi = prm->bc_xhi; c->g.bylo = prm->bc_ylo; c->g.byhi = prm->bc_yhi;
   c->g.nnx = (prm->bc_xlo == NH_BC_PERIODIC) ? nx : nx + 1;
   c->g.nny = (prm->bc_ylo == NH_BC_PERIODIC) ? ny : ny + 1;
-  c->g.np = nx + 1;
+  c->g.np = nh_node_pitch(c->g.nnx);
   c->prm = *prm;
   c->stream = (cudaStream_t)cuda_stream;
   c->device = dev;
   c->sm_count = prop.multiProcessorCount;
   c->nc = (size_t)nx * ny;
   c->nn = (size_t)(nx + 1) * (ny + 1);
+  c->nni = (size_t)c->g.np * (ny + 1 + 2 * NH_ROW_PAD);
   c->cur = 0; c->curw = 0;
   c->lam_valid = false;
   c->host_status = NH_OK;
@@ -231,13 +256,14 @@ int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* 
   double** cells[] = {&c->H, &c->h[0], &c->h[1], &c->h[2], &c->qx[0], &c->qx[1], &c->qx[2],
                       &c->qy[0], &c->qy[1], &c->qy[2], &c->qx1, &c->qy1, &c->z};
   double** nodes[] = {&c->w[0], &c->w[1], &c->w[2], &c->p, &c->b, &c->dg, &c->dinv, &c->cE, &c->cW,
-                      &c->cN, &c->cS, &c->ky, &c->kr, &c->kr0, &c->kpA, &c->kpB, &c->kvA, &c->kvB,
-                      &c->kt, &c->w2};
+                      &c->cN, &c->cS, &c->ky, &c->kr, &c->krB, &c->kr0, &c->kpA, &c->kpB, &c->kvA,
+                      &c->kvB, &c->kt, &c->w2};
   for (double** p : cells) ok = ok && dalloc(c, p, c->nc);
-  for (double** p : nodes) ok = ok && dalloc(c, p, c->nn);
+  for (double** p : nodes) ok = ok && nalloc(c, p);
+  ok = ok && dalloc(c, &c->pub, c->nn);
   if (prm->breaking) {
     ok = ok && dalloc(c, &c->qx2, c->nc) && dalloc(c, &c->qy2, c->nc);
-    ok = ok && dalloc(c, &c->flag_c, c->nc) && dalloc(c, &c->flag_n, c->nn);
+    ok = ok && dalloc(c, &c->flag_c, c->nc) && dalloc(c, &c->flag_n, c->nni);
   }
   ok = ok && dalloc(c, &c->sc, 1);
   if (ok && cudaMallocHost((void**)&c->sc_host, sizeof(NhScal)) != cudaSuccess) ok = false;
@@ -272,7 +298,7 @@ int nh_set_state(nh_ctx* c, const double* h, const double* qx, const double* qy,
                  const double* p) {
   if (!c || !h || !qx || !qy) return NH_EINVAL;
   int s1, s2; other_slots(c->cur, s1, s2);
-  size_t cb = c->nc * sizeof(double), nb = c->nn * sizeof(double);
+  size_t cb = c->nc * sizeof(double);
   // stage into a free slot, validate there, then make it current (an invalid state changes nothing)
   if (copy_async(c, c->h[s1], h, cb) || copy_async(c, c->qx[s1], qx, cb) ||
       copy_async(c, c->qy[s1], qy, cb))
@@ -285,19 +311,16 @@ int nh_set_state(nh_ctx* c, const double* h, const double* qx, const double* qy,
   if (c->sc_host->flags & NH_FLAG_BADSTATE)
     return fail(c, NH_EINVAL, "set_state: h<0 or non-finite input");
   c->cur = s1;
-  if (w) { if (copy_async(c, c->w[c->curw], w, nb)) return NH_ECUDA; }
-  else cudaMemsetAsync(c->w[c->curw], 0, nb, c->stream);
-  if (p) { if (copy_async(c, c->p, p, nb)) return NH_ECUDA; }
-  else cudaMemsetAsync(c->p, 0, nb, c->stream);
+  if (node_in(c, c->w[c->curw], w) || node_in(c, c->p, p)) return NH_ECUDA;
   c->lam_valid = false;
   return NH_OK;
 }
 
-// node array out in the public layout (periodic duplicate lines filled), via scratch
-static int node_out(nh_ctx* c, const double* src, double* dst_user, double* scratch) {
-  nh_launch_nodes_out(c, src, scratch);
+// node plane out in the public layout (periodic duplicate lines filled), via the dense staging plane
+static int node_out(nh_ctx* c, const double* src, double* dst_user) {
+  nh_launch_nodes_out(c, src, c->pub);
   if (check_launch(c) != NH_OK) return NH_ECUDA;
-  return copy_async(c, dst_user, scratch, c->nn * sizeof(double));
+  return copy_async(c, dst_user, c->pub, c->nn * sizeof(double));
 }
 
 int nh_get_state(nh_ctx* c, double* h, double* qx, double* qy, double* w, double* p) {
@@ -306,9 +329,8 @@ int nh_get_state(nh_ctx* c, double* h, double* qx, double* qy, double* w, double
   if (h && copy_async(c, h, c->h[c->cur], cb)) return NH_ECUDA;
   if (qx && copy_async(c, qx, c->qx[c->cur], cb)) return NH_ECUDA;
   if (qy && copy_async(c, qy, c->qy[c->cur], cb)) return NH_ECUDA;
-  // kt / kr are solver scratch, free between solves
-  if (w && node_out(c, c->w[c->curw], w, c->kt)) return NH_ECUDA;
-  if (p && node_out(c, c->p, p, c->kr)) return NH_ECUDA;
+  if (w && node_out(c, c->w[c->curw], w)) return NH_ECUDA;
+  if (p && node_out(c, c->p, p)) return NH_ECUDA;
   cudaError_t e = cudaStreamSynchronize(c->stream);
   if (e != cudaSuccess) { c->host_status = NH_ECUDA; return fail(c, NH_ECUDA, cudaGetErrorString(e)); }
   return NH_OK;
@@ -437,10 +459,10 @@ int nh_compute_dt(nh_ctx* c, double* dt_host) {
 
 int nh_apply_A(nh_ctx* c, const double* x_nodes, double* y_nodes) {
   if (!c || !x_nodes || !y_nodes) return NH_EINVAL;
-  if (copy_async(c, c->kpA, x_nodes, c->nn * sizeof(double))) return NH_ECUDA;
+  if (node_in(c, c->kpA, x_nodes)) return NH_ECUDA;
   nh_launch_compute_z(c, c->h[c->cur], c->z);
   nh_launch_apply_A(c, c->h[c->cur], c->z, c->kpA, c->kpB);
-  if (node_out(c, c->kpB, y_nodes, c->kvA)) return NH_ECUDA;
+  if (node_out(c, c->kpB, y_nodes)) return NH_ECUDA;
   cudaStreamSynchronize(c->stream);
   return check_launch(c);
 }
@@ -452,7 +474,7 @@ int nh_coeffs(nh_ctx* c, double* AC, double* AE, double* AW, double* AN, double*
   const double* src[5] = {c->dg, c->cE, c->cW, c->cN, c->cS};
   double* dst[5] = {AC, AE, AW, AN, AS};
   for (int k = 0; k < 5; ++k)
-    if (node_out(c, src[k], dst[k], c->kvA)) return NH_ECUDA;
+    if (node_out(c, src[k], dst[k])) return NH_ECUDA;
   cudaStreamSynchronize(c->stream);
   return check_launch(c);
 }
@@ -462,7 +484,7 @@ static int rhs_hook(nh_ctx* c, double dt, double* out, int constraint_only) {
   nh_launch_compute_z(c, c->h[c->cur], c->z);
   nh_launch_rhs(c, c->h[c->cur], c->qx[c->cur], c->qy[c->cur], c->z, c->w[c->curw], c->b,
                 constraint_only);
-  if (node_out(c, c->b, out, c->kvA)) return NH_ECUDA;
+  if (node_out(c, c->b, out)) return NH_ECUDA;
   cudaStreamSynchronize(c->stream);
   return check_launch(c);
 }
@@ -477,13 +499,12 @@ int nh_constraint(nh_ctx* c, double* B_nodes) {
 
 int nh_solve(nh_ctx* c, const double* b_nodes, double* x_nodes, int* iters, double* relres) {
   if (!c || !b_nodes || !x_nodes) return NH_EINVAL;
-  size_t nb = c->nn * sizeof(double);
-  if (copy_async(c, c->b, b_nodes, nb) || copy_async(c, c->w2, x_nodes, nb)) return NH_ECUDA;
+  if (node_in(c, c->b, b_nodes) || node_in(c, c->w2, x_nodes)) return NH_ECUDA;
   nh_launch_compute_z(c, c->h[c->cur], c->z);
   nh_launch_coeffs(c, c->h[c->cur], c->z);
   nh_launch_scale_coeffs(c);
   nh_launch_solve(c, c->b, c->w2, 0);
-  if (node_out(c, c->w2, x_nodes, c->kvA)) return NH_ECUDA;
+  if (node_out(c, c->w2, x_nodes)) return NH_ECUDA;
   if (check_launch(c) != NH_OK) return NH_ECUDA;
   if (read_scalars(c) != NH_OK) return NH_ECUDA;
   if (iters) *iters = c->sc_host->iters_last;

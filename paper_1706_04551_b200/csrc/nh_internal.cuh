@@ -21,7 +21,7 @@
 struct NhGrid {
   int nx, ny;    // cells
   int nnx, nny;  // distinct node lines: n in a periodic direction, n+1 otherwise
-  int np;        // node pitch = nx+1 (public node layout, kept internally)
+  int np;        // internal node pitch (even; >= nnx + 4: two ghost / padding columns on each side)
   int bxlo, bxhi, bylo, byhi;
   double dx, dy;
 };
@@ -95,6 +95,13 @@ __device__ __forceinline__ double nh_minmod(double a, double b) {
   return (a > 0.0) ? fmin(a, b) : fmax(a, b);
 }
 
+// Internal node planes: pitch NP = 60 * ceil(nnx / 60) + 4 doubles, ny + 5 rows; the pointer
+// handed to kernels addresses node (0,0) = physical element (2 rows, 2 columns), so that
+// a[J * np + I] is valid for -2 <= I < np - 2 and -2 <= J <= ny + 2: ghost lines need no index map
+// and every even column is 16-byte aligned (nh_solver.cu).
+constexpr int NH_STRIP = 60, NH_ROW_PAD = 2;
+inline int nh_node_pitch(int nnx) { return NH_STRIP * ((nnx + NH_STRIP - 1) / NH_STRIP) + 4; }
+
 // ---- context ------------------------------------------------------------------------------
 struct nh_ctx {
   NhGrid g;
@@ -121,9 +128,12 @@ struct nh_ctx {
   double* p;   // pressure multiplier p~ (warm start of the next solve)
   double* b;   // right-hand side
   double *dg, *dinv, *cE, *cW, *cN, *cS;  // diag(A), its inverse, column-scaled off-diagonals
-  double *ky, *kr, *kr0, *kpA, *kpB, *kvA, *kvB, *kt;  // BiCGStab vectors
+  double *ky, *kr, *krB, *kr0, *kpA, *kpB, *kvA, *kvB, *kt;  // BiCGStab vectors (r, p, v double-buffered)
+  double* pub;   // dense (nx+1) x (ny+1) staging plane for the public node layout
+  std::vector<void*> raw;  // allocation bases (node planes are handed out offset to node (0,0))
   double* part;  // per-CTA partial sums of the solver
-  int solver_grid, solver_occ;
+  int solver_grid, solver_occ, solver_nstrips, solver_R, solver_nbands;
+  size_t nni;  // doubles per internal node plane (ghost ring included)
   NhScal* sc;       // device scalars
   NhScal* sc_host;  // pinned mirror
   int cur;          // index of the cell slot (h, qx, qy) holding the current state
@@ -150,7 +160,7 @@ void nh_launch_breaking(nh_ctx* c, const double* h, const double* qx1, const dou
 void nh_launch_rhs(nh_ctx* c, const double* h, const double* qx, const double* qy, const double* z,
                    const double* w, double* b, int constraint_only);
 void nh_launch_coeffs(nh_ctx* c, const double* h, const double* z);  // -> dg, dinv, raw cE..cS
-void nh_launch_scale_coeffs(nh_ctx* c);                              // cX *= dinv(neighbour)
+void nh_launch_scale_coeffs(nh_ctx* c);  // cX *= dinv(neighbour); ghost lines <- (swapped) images
 void nh_launch_apply_A(nh_ctx* c, const double* h, const double* z, const double* x, double* y);
 void nh_launch_correct(nh_ctx* c, const double* h, const double* z, const double* qx2,
                        const double* qy2, const double* w2, const double* p, double* qx_out,

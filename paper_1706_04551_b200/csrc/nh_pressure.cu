@@ -331,14 +331,14 @@ k_relax(NhGrid G, const NhScal* sc, int stage, double g, double A, double h0, do
   }
 }
 
-// public node layout out: fill the duplicate lines of periodic directions
+// internal plane -> dense public node layout: fill the duplicate lines of periodic directions
 __global__ void __launch_bounds__(BX* BY)
 k_nodes_out(NhGrid G, const double* __restrict__ src, double* __restrict__ dst) {
   int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
   if (I > G.nx || J > G.ny) return;
   int II = (I == G.nx && G.nnx == G.nx) ? 0 : I;
   int JJ = (J == G.ny && G.nny == G.ny) ? 0 : J;
-  dst[(size_t)J * G.np + I] = src[(size_t)JJ * G.np + II];
+  dst[(size_t)J * (G.nx + 1) + I] = src[(size_t)JJ * G.np + II];
 }
 
 dim3 grid2(int nx, int ny) { return dim3((nx + BX - 1) / BX, (ny + BY - 1) / BY); }

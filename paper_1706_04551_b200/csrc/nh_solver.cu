@@ -280,3 +280,222 @@ __device__ void pass_CA(const SolveP& P, double alpha, double omega, double beta
   }
   block_partials<2>(acc, P.part, buf, red);
 }
+
+// ---- simple phases (a handful per solve): rows over CTAs, columns over threads --------------
+// y = dg * x at the real nodes, with ghost images
+__device__ void phase_y_from_x(const SolveP& P) {
+  const NhGrid& G = P.G;
+  for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
+    for (int I = threadIdx.x; I < G.nnx; I += NT) {
+      size_t k = nidx(G, I, J);
+      store_images(G, P.y, I, J, P.x[k] * P.dg[k]);
+    }
+}
+
+// true residual r = b - (A M^-1) y, r0 = r (S9: the true residual decides); partials r.r, b.b
+__device__ void phase_init(const SolveP& P, double* r, int buf, double (*red)[NW]) {
+  const NhGrid& G = P.G;
+  double acc[2] = {0.0, 0.0};
+  for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
+    for (int I = threadIdx.x; I < G.nnx; I += NT) {
+      size_t k = nidx(G, I, J);
+      const double* y = P.y;
+      double ay = y[k] + P.cE[k] * y[k + 1] + P.cW[k] * y[k - 1] + P.cN[k] * y[k + G.np] +
+                  P.cS[k] * y[k - G.np];
+      double bb = P.b[k];
+      double rr = bb - ay;
+      store_images(G, r, I, J, rr);
+      P.r0[k] = rr;
+      acc[0] += rr * rr; acc[1] += bb * bb;
+    }
+  block_partials<2>(acc, P.part, buf, red);
+}
+
+// y += alpha p + omega s, s = r - alpha v  (final update of an iteration whose pass CA never ran:
+// half-step exit with omega = 0, and the polish iteration)
+__device__ void phase_update_y(const SolveP& P, double alpha, double omega, const double* r,
+                               const double* p, const double* v) {
+  const NhGrid& G = P.G;
+  for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
+    for (int I = threadIdx.x; I < G.nnx; I += NT) {
+      size_t k = nidx(G, I, J);
+      double s = r[k] - alpha * v[k];
+      store_images(G, P.y, I, J, P.y[k] + (alpha * p[k] + omega * s));
+    }
+}
+
+// x = M^-1 y  (or zeros when b = 0)
+__device__ void phase_out(const SolveP& P, bool zero) {
+  const NhGrid& G = P.G;
+  for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
+    for (int I = threadIdx.x; I < G.nnx; I += NT) {
+      size_t k = nidx(G, I, J);
+      P.x[k] = zero ? 0.0 : P.y[k] * P.dinv[k];
+    }
+}
+
+__global__ void __launch_bounds__(NT, 2) k_bicgstab(SolveP P) {
+  cg::grid_group grid = cg::this_grid();
+  __shared__ double red[MAXDOT][NW];
+  __shared__ double bc[MAXDOT];
+
+  double *rC = P.rA, *rN = P.rB, *pC = P.pA, *pN = P.pB, *vC = P.vA, *vN = P.vB;  // current / next
+  auto flip = [&]() {
+    double* t;
+    t = rC; rC = rN; rN = t;
+    t = pC; pC = pN; pN = t;
+    t = vC; vC = vN; vN = t;
+  };
+  int buf = 0;  // partial buffer of the pass in flight (alternates: one grid barrier per pass)
+  int iters = 0, converged = 0, status = 0;
+  double rnorm = 0.0, bnorm = 0.0, tol = 0.0;
+
+  phase_y_from_x(P);
+  grid.sync();
+  for (int cycle = 0; cycle < 8 && !converged; ++cycle) {
+    double d2[2], d5[5];
+    phase_init(P, rC, buf, red);
+    grid.sync();
+    grid_sums<2>(P.part, buf, d2, red, bc);
+    buf ^= 1;
+    rnorm = sqrt(d2[0]);
+    if (cycle == 0) {
+      bnorm = sqrt(d2[1]);
+      if (!(bnorm == bnorm) || isinf(bnorm)) { status = NH_ENAN; break; }
+      if (bnorm == 0.0) break;
+      tol = P.rtol * bnorm;
+    }
+    if (!(rnorm == rnorm)) { status = NH_ENAN; break; }
+    if (rnorm <= tol) { converged = 1; break; }
+    if (iters >= P.maxit) break;
+    // first direction of the cycle: p = r, v = (A M^-1) p, sigma = r0.v
+    double rho = d2[0];
+    pass_CA<true>(P, 0.0, 0.0, 0.0, rC, pC, vC, rN, pN, vN, buf, red);
+    flip();
+    grid.sync();
+    grid_sums<2>(P.part, buf, d2, red, bc);
+    buf ^= 1;
+    double sigma = d2[0];
+    while (iters < P.maxit) {
+      if (fabs(rho) < 1e-300 || fabs(sigma) < 1e-300) break;  // breakdown -> restart
+      double alpha = rho / sigma;
+      iters++;
+      pass_B(P, alpha, rC, vC, buf, red);
+      grid.sync();
+      grid_sums<5>(P.part, buf, d5, red, bc);
+      buf ^= 1;
+      if (sqrt(d5[2]) <= tol) {  // half-step exit: x += alpha p^
+        phase_update_y(P, alpha, 0.0, rC, pC, vC);
+        grid.sync();
+        break;
+      }
+      if (d5[1] == 0.0) break;
+      double omega = d5[0] / d5[1];
+      if (fabs(omega) < 1e-300 || !(omega == omega)) break;
+      double rho_new = d5[3] - omega * d5[4];  // r0.r' = r0.s - omega r0.t  (R25)
+      double beta = (rho_new / rho) * (alpha / omega);
+      rho = rho_new;
+      pass_CA<false>(P, alpha, omega, beta, rC, pC, vC, rN, pN, vN, buf, red);
+      flip();
+      grid.sync();
+      grid_sums<2>(P.part, buf, d2, red, bc);
+      buf ^= 1;
+      sigma = d2[0];
+      rnorm = sqrt(d2[1]);
+      if (!(rnorm == rnorm)) break;
+      if (rnorm <= tol) break;
+    }
+    // loop back: the true residual decides (the recursive residual may have drifted)
+  }
+  if (status == 0 && bnorm > 0.0 && !converged) status = NH_ENOCONV;
+
+  // one extra "polish" iteration from the true residual (R14): r0 = r, p = r
+  if (converged && rnorm > 0.0) {
+    double d2[2], d5[5];
+    double rho = rnorm * rnorm;
+    pass_CA<true>(P, 0.0, 0.0, 0.0, rC, pC, vC, rN, pN, vN, buf, red);
+    flip();
+    grid.sync();
+    grid_sums<2>(P.part, buf, d2, red, bc);
+    buf ^= 1;
+    double sigma = d2[0];
+    if (fabs(rho) >= 1e-300 && fabs(sigma) >= 1e-300) {
+      double alpha = rho / sigma;
+      pass_B(P, alpha, rC, vC, buf, red);
+      grid.sync();
+      grid_sums<5>(P.part, buf, d5, red, bc);
+      buf ^= 1;
+      double omega = (d5[1] > 0.0) ? d5[0] / d5[1] : 0.0;
+      phase_update_y(P, alpha, omega, rC, pC, vC);
+      grid.sync();
+    }
+  }
+  if (status != NH_ENAN) phase_out(P, bnorm == 0.0);
+
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    NhScal* sc = P.sc;
+    if (status == NH_ENOCONV) sc->flags |= NH_FLAG_NOCONV;
+    if (status == NH_ENAN) sc->flags |= NH_FLAG_NAN;
+    sc->iters_last = iters;
+    sc->res_last = (bnorm > 0.0) ? rnorm / bnorm : 0.0;
+    if (P.count_stats) {
+      sc->iters_total += iters;
+      sc->solves += 1;
+      if (iters > sc->iters_max) sc->iters_max = iters;
+    }
+  }
+}
+
+}  // namespace
+
+// Cooperative grid (one wave of co-resident CTAs) and the band height R: every warp takes the
+// units u = gw, gw + tw, ... (strip fastest, so neighbouring warps sweep neighbouring strips of the
+// same band); R minimises rounds x (R + 2 halo rows).
+int nh_solver_setup(nh_ctx* c) {
+  int occ = 0;
+  cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bicgstab, NT, 0);
+  if (e != cudaSuccess || occ < 1) {
+    snprintf(c->err, sizeof(c->err), "solver occupancy query failed: %s", cudaGetErrorString(e));
+    return NH_ECUDA;
+  }
+  const int nnx = c->g.nnx, nny = c->g.nny;
+  const int nstrips = (nnx + SW - 1) / SW;
+  long long small_units = (long long)nstrips * ((nny + 7) / 8);
+  long long grid = (long long)occ * c->sm_count;
+  if (grid > (small_units + NW - 1) / NW) grid = (small_units + NW - 1) / NW;
+  if (grid < 1) grid = 1;
+  const long long tw = grid * NW;
+  int bestR = nny;
+  long long best = -1;
+  for (int R = 4; R <= nny; ++R) {
+    long long nb = (nny + R - 1) / R;
+    long long rounds = (nstrips * nb + tw - 1) / tw;
+    long long cost = rounds * (R + 2);
+    if (best < 0 || cost < best) { best = cost; bestR = R; }
+  }
+  if (nny < 4) bestR = nny;
+  c->solver_occ = occ;
+  c->solver_grid = (int)grid;
+  c->solver_nstrips = nstrips;
+  c->solver_R = bestR;
+  c->solver_nbands = (nny + bestR - 1) / bestR;
+  e = cudaMalloc(&c->part, sizeof(double) * 2 * MAXDOT * (size_t)grid);
+  if (e != cudaSuccess) return NH_ENOMEM;
+  return NH_OK;
+}
+
+void nh_launch_solve(nh_ctx* c, const double* b, double* x, int count_stats) {
+  SolveP P;
+  P.G = c->g;
+  P.nstrips = c->solver_nstrips; P.R = c->solver_R; P.nbands = c->solver_nbands;
+  P.cE = c->cE; P.cW = c->cW; P.cN = c->cN; P.cS = c->cS; P.dg = c->dg; P.dinv = c->dinv;
+  P.b = b; P.x = x;
+  P.y = c->ky; P.r0 = c->kr0; P.t = c->kt;
+  P.rA = c->kr; P.rB = c->krB; P.pA = c->kpA; P.pB = c->kpB; P.vA = c->kvA; P.vB = c->kvB;
+  P.part = c->part; P.sc = c->sc; P.rtol = c->prm.solver_rtol; P.maxit = c->prm.solver_maxit;
+  P.count_stats = count_stats;
+  void* args[] = {&P};
+  NH_CUDA_OK(c, cudaLaunchCooperativeKernel((void*)k_bicgstab, dim3(c->solver_grid), dim3(NT), args,
+                                            0, c->stream));
+  c->launches++;
+}
