@@ -683,7 +683,8 @@ static int nonhydro_part(nho_ctx* c, const double* w_in, double dt, double* qx_o
 #pragma omp parallel for if (c->ny >= 48) schedule(static)
   for (int J = 0; J < c->nny; ++J)
     for (int I = 0; I < c->nnx; ++I)
-      c->b[NIDX(c, I, J)] = -node_B(c, c->h1, c->qx2, c->qy2, c->z, c->w2, I, J) / dt;
+      c->b[NIDX(c, I, J)] = (dt > 0.0) ? -node_B(c, c->h1, c->qx2, c->qy2, c->z, c->w2, I, J) / dt
+                                       : 0.0;   /* R26: all-dry domain, dt = 0 => p~ = 0 */
   int iters = 0; double relres = 0.0;
   int st = bicgstab(c, c->h1, c->z, c->b, c->p, &iters, &relres);
   c->info.iters_last = iters;

@@ -156,7 +156,8 @@ k_rhs(NhGrid G, const NhScal* sc, int constraint_only, const double* __restrict_
   size_t k = (size_t)J * G.np + I;
   double B = hn * divq - 0.5 * (q1E + q1W) * (zE - zW) / G.dx -
              0.5 * (q2N + q2S) * (zN - zS) / G.dy + 2.0 * hn * w[k];
-  b[k] = constraint_only ? B : -B / sc->dt;
+  const double dt = sc->dt;
+  b[k] = constraint_only ? B : ((dt > 0.0) ? -B / dt : 0.0);  // R26: dt = 0 (all dry) => b = 0
 }
 
 // S6: breaking sources at cells (section 3, eqs (9)-(12); 2D reading R12): q** = q* + dt R_u
