@@ -44,7 +44,13 @@ namespace cg = cooperative_groups;
 
 namespace {
 
-constexpr int NT = 256, NW = NT / 32;  // CTA size, warps per CTA
+#ifndef NH_NT
+#define NH_NT 256
+#endif
+#ifndef NH_MINB
+#define NH_MINB 2
+#endif
+constexpr int NT = NH_NT, NW = NT / 32;  // CTA size, warps per CTA
 constexpr int SW = 60;                 // owned columns per warp strip
 constexpr int MAXDOT = 5;
 
@@ -159,8 +165,26 @@ __device__ __forceinline__ Unit make_unit(const SolveP& P, int u, int lane) {
   return U;
 }
 
+// 16-byte load of the lane's column pair of row j
+#ifndef NH_LD
+#define NH_LD 0
+#endif
 __device__ __forceinline__ double2 ld2(const double* a, const NhGrid& G, int c0, int j) {
+#if NH_LD == 1
+  return __ldcg(reinterpret_cast<const double2*>(a + nidx(G, c0, j)));
+#elif NH_LD == 2
+  return __ldcs(reinterpret_cast<const double2*>(a + nidx(G, c0, j)));
+#else
   return *reinterpret_cast<const double2*>(a + nidx(G, c0, j));
+#endif
+}
+// planes that no pass of the kernel writes (the column-scaled off-diagonals)
+__device__ __forceinline__ double2 ld2c(const double* a, const NhGrid& G, int c0, int j) {
+#if NH_LDC == 1
+  return __ldg(reinterpret_cast<const double2*>(a + nidx(G, c0, j)));
+#else
+  return ld2(a, G, c0, j);
+#endif
 }
 
 // store the lane's pair of row j (owned columns only), with ghost images on boundary nodes
@@ -177,24 +201,57 @@ __device__ __forceinline__ void st2(double* a, const SolveP& P, const Unit& U, i
   }
 }
 
+// Register-resident operands of one sweep row.  Every pass is software-pipelined by hand: the
+// loads of the NEXT row are issued before the current row is computed and stored (the compiler
+// cannot hoist them itself across the stores of possibly aliasing planes), so each warp keeps one
+// full row of every plane (~3-5 KB) in flight while it computes.
+struct RowC {  // coefficient row j of (A M^-1) and the shadow residual
+  double2 q, e, w, n, s;
+};
+__device__ __forceinline__ RowC ld_rowc(const SolveP& P, int c0, int j) {
+  RowC C;
+  C.q = ld2(P.r0, P.G, c0, j);
+  C.e = ld2c(P.cE, P.G, c0, j); C.w = ld2c(P.cW, P.G, c0, j);
+  C.n = ld2c(P.cN, P.G, c0, j); C.s = ld2c(P.cS, P.G, c0, j);
+  return C;
+}
+
 // (A M^-1) applied to the operand rows (m: j-1, c: j, n: j+1) at the lane's two columns of row j
-__device__ __forceinline__ double2 stencil2(const SolveP& P, int c0, int j, double2 m, double2 c,
-                                            double2 n) {
-  const NhGrid& G = P.G;
-  double2 e = ld2(P.cE, G, c0, j), w = ld2(P.cW, G, c0, j);
-  double2 nn = ld2(P.cN, G, c0, j), ss = ld2(P.cS, G, c0, j);
+__device__ __forceinline__ double2 stencil2(const RowC& C, double2 m, double2 c, double2 n) {
   double west0 = __shfl_up_sync(0xffffffffu, c.y, 1);
   double east1 = __shfl_down_sync(0xffffffffu, c.x, 1);
   double2 o;
-  o.x = fma(ss.x, m.x, fma(nn.x, n.x, fma(w.x, west0, fma(e.x, c.y, c.x))));
-  o.y = fma(ss.y, m.y, fma(nn.y, n.y, fma(w.y, c.x, fma(e.y, east1, c.y))));
+  o.x = fma(C.s.x, m.x, fma(C.n.x, n.x, fma(C.w.x, west0, fma(C.e.x, c.y, c.x))));
+  o.y = fma(C.s.y, m.y, fma(C.n.y, n.y, fma(C.w.y, c.x, fma(C.e.y, east1, c.y))));
   return o;
 }
 
+#if defined(NH_NOINLINE)
+#define NH_PASS_INLINE __noinline__
+#else
+#define NH_PASS_INLINE __forceinline__
+#endif
+#ifndef NH_PF_B
+#define NH_PF_B 1
+#endif
+#ifndef NH_PF_CA
+#define NH_PF_CA 0
+#endif
+
 // pass B: s = r - alpha v (rows Ja-1..Jb), t = (A M^-1) s (rows Ja..Jb-1);
 // partials: t.s, t.t, s.s, r0.s, r0.t
-__device__ void pass_B(const SolveP& P, double alpha, const double* r, const double* v, int buf,
-                       double (*red)[NW]) {
+struct RowB {  // operands of one sweep step of pass B: vectors of row j+1, coefficients of row j
+  double2 r, v;
+  RowC C;
+};
+__device__ __forceinline__ void ld_rowb(RowB& X, const SolveP& P, const double* r, const double* v,
+                                        int c0, int jv, int jc) {
+  X.r = ld2(r, P.G, c0, jv); X.v = ld2(v, P.G, c0, jv);
+  X.C = ld_rowc(P, c0, jc);
+}
+
+__device__ NH_PASS_INLINE void pass_B(const SolveP& P, double alpha, const double* r, const double* v,
+                                    int buf, double (*red)[NW]) {
   const NhGrid& G = P.G;
   const int lane = threadIdx.x & 31;
   const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
@@ -202,17 +259,20 @@ __device__ void pass_B(const SolveP& P, double alpha, const double* r, const dou
   double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
   for (int u = gw; u < nunits; u += tw) {
     Unit U = make_unit(P, u, lane);
-    auto srow = [&](int j) {
-      double2 a = ld2(r, G, U.c0, j), b = ld2(v, G, U.c0, j);
+    auto srow = [&](double2 a, double2 b) {
       return make_double2(fma(-alpha, b.x, a.x), fma(-alpha, b.y, a.y));
     };
-    double2 sm = srow(U.Ja - 1), sc = srow(U.Ja);
-#pragma unroll 2
-    for (int j = U.Ja; j < U.Jb; ++j) {
-      double2 sn = srow(j + 1);
-      double2 q = ld2(P.r0, G, U.c0, j);
-      double2 t = stencil2(P, U.c0, j, sm, sc, sn);
+    double2 sm = srow(ld2(r, G, U.c0, U.Ja - 1), ld2(v, G, U.c0, U.Ja - 1));
+    double2 sc = srow(ld2(r, G, U.c0, U.Ja), ld2(v, G, U.c0, U.Ja));
+    // one sweep step: row j from the operand set `cur`; the set of the next step is requested
+    // first (`nxt`; row indices clamped, the last request is never used)
+    auto step = [&](int j, RowB& cur, RowB& nxt) {
+      if (NH_PF_B) ld_rowb(nxt, P, r, v, U.c0, min(j + 2, U.Jb), min(j + 1, U.Jb - 1));
+      else ld_rowb(cur, P, r, v, U.c0, j + 1, j);
+      double2 sn = srow(cur.r, cur.v);
+      double2 t = stencil2(cur.C, sm, sc, sn);
       st2(P.t, P, U, j, t);
+      const double2 q = cur.C.q;
       if (U.own0) {
         acc[0] = fma(t.x, sc.x, acc[0]); acc[1] = fma(t.x, t.x, acc[1]); acc[2] = fma(sc.x, sc.x, acc[2]);
         acc[3] = fma(q.x, sc.x, acc[3]); acc[4] = fma(q.x, t.x, acc[4]);
@@ -222,6 +282,12 @@ __device__ void pass_B(const SolveP& P, double alpha, const double* r, const dou
         acc[3] = fma(q.y, sc.y, acc[3]); acc[4] = fma(q.y, t.y, acc[4]);
       }
       sm = sc; sc = sn;
+    };
+    RowB A, B;
+    if (NH_PF_B) ld_rowb(A, P, r, v, U.c0, U.Ja + 1, U.Ja);
+    for (int j = U.Ja; j < U.Jb; j += 2) {  // ping-pong operand sets: no register rotation
+      step(j, A, B);
+      if (j + 1 < U.Jb) step(j + 1, B, A);
     }
   }
   block_partials<5>(acc, P.part, buf, red);
@@ -229,32 +295,48 @@ __device__ void pass_B(const SolveP& P, double alpha, const double* r, const dou
 
 // pass CA: FIRST: p' = r' = r (start of a cycle).  Otherwise s = r - alpha v; y += alpha p + omega s;
 // r' = s - omega t; p' = r' + beta (p - omega v).  Then v' = (A M^-1) p'.  partials: r0.v', r'.r'
+struct RowV {  // vector row of pass CA
+  double2 r, v, t, p, y;
+};
 template <bool FIRST>
-__device__ void pass_CA(const SolveP& P, double alpha, double omega, double beta, const double* r,
-                        const double* p, const double* v, double* rN, double* pN, double* vN,
-                        int buf, double (*red)[NW]) {
-  const NhGrid& G = P.G;
+__device__ __forceinline__ void ld_rowv(RowV& V, const SolveP& P, const double* r, const double* p,
+                                        const double* v, int c0, int j) {
+  V.r = ld2(r, P.G, c0, j);
+  if (!FIRST) {
+    V.v = ld2(v, P.G, c0, j); V.t = ld2(P.t, P.G, c0, j);
+    V.p = ld2(p, P.G, c0, j); V.y = ld2(P.y, P.G, c0, j);
+  }
+}
+struct RowCA {  // operands of one sweep step of pass CA: vectors of row j+1, coefficients of row j
+  RowV V;
+  RowC C;
+};
+
+template <bool FIRST>
+__device__ NH_PASS_INLINE void pass_CA(const SolveP& P, double alpha, double omega, double beta,
+                                     const double* r, const double* p, const double* v, double* rN,
+                                     double* pN, double* vN, int buf, double (*red)[NW]) {
   const int lane = threadIdx.x & 31;
   const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
   const int nunits = P.nstrips * P.nbands;
   double acc[2] = {0.0, 0.0};
   for (int u = gw; u < nunits; u += tw) {
     Unit U = make_unit(P, u, lane);
-    // new p of row j; on owned rows also the y / r' / p' stores and the r'.r' partial
-    auto prow = [&](int j, bool owned_row) {
-      double2 a = ld2(r, G, U.c0, j);
+    // new p of row j from its loaded operands; on owned rows also the y / r' / p' stores and the
+    // r'.r' partial
+    auto prow = [&](const RowV& V, int j, bool owned_row) {
       double2 rn, pn;
       if (FIRST) {
-        rn = a; pn = a;
+        rn = V.r; pn = V.r;
       } else {
-        double2 b = ld2(v, G, U.c0, j), c = ld2(P.t, G, U.c0, j), d = ld2(p, G, U.c0, j);
-        double2 s = make_double2(fma(-alpha, b.x, a.x), fma(-alpha, b.y, a.y));
-        rn = make_double2(fma(-omega, c.x, s.x), fma(-omega, c.y, s.y));
-        pn = make_double2(fma(beta, fma(-omega, b.x, d.x), rn.x), fma(beta, fma(-omega, b.y, d.y), rn.y));
+        double2 s = make_double2(fma(-alpha, V.v.x, V.r.x), fma(-alpha, V.v.y, V.r.y));
+        rn = make_double2(fma(-omega, V.t.x, s.x), fma(-omega, V.t.y, s.y));
+        pn = make_double2(fma(beta, fma(-omega, V.v.x, V.p.x), rn.x),
+                          fma(beta, fma(-omega, V.v.y, V.p.y), rn.y));
         if (owned_row) {
-          double2 yy = ld2(P.y, G, U.c0, j);
-          yy.x = yy.x + fma(omega, s.x, alpha * d.x);
-          yy.y = yy.y + fma(omega, s.y, alpha * d.y);
+          double2 yy;
+          yy.x = V.y.x + fma(omega, s.x, alpha * V.p.x);
+          yy.y = V.y.y + fma(omega, s.y, alpha * V.p.y);
           st2(P.y, P, U, j, yy);
         }
       }
@@ -266,16 +348,33 @@ __device__ void pass_CA(const SolveP& P, double alpha, double omega, double beta
       }
       return pn;
     };
-    double2 pm = prow(U.Ja - 1, false), pc = prow(U.Ja, true);
-#pragma unroll 2
-    for (int j = U.Ja; j < U.Jb; ++j) {
-      double2 pn = prow(j + 1, j + 1 < U.Jb);
-      double2 q = ld2(P.r0, G, U.c0, j);
-      double2 vv = stencil2(P, U.c0, j, pm, pc, pn);
+    double2 pm, pc;
+    {
+      RowV V0, V1;
+      ld_rowv<FIRST>(V0, P, r, p, v, U.c0, U.Ja - 1);
+      ld_rowv<FIRST>(V1, P, r, p, v, U.c0, U.Ja);
+      pm = prow(V0, U.Ja - 1, false);
+      pc = prow(V1, U.Ja, true);
+    }
+    auto ld_set = [&](RowCA& X, int jv, int jc) {
+      ld_rowv<FIRST>(X.V, P, r, p, v, U.c0, jv);
+      X.C = ld_rowc(P, U.c0, jc);
+    };
+    auto step = [&](int j, RowCA& cur, RowCA& nxt) {
+      if (NH_PF_CA) ld_set(nxt, min(j + 2, U.Jb), min(j + 1, U.Jb - 1));
+      else ld_set(cur, j + 1, j);
+      double2 pn = prow(cur.V, j + 1, j + 1 < U.Jb);
+      double2 vv = stencil2(cur.C, pm, pc, pn);
       st2(vN, P, U, j, vv);
-      if (U.own0) acc[0] = fma(q.x, vv.x, acc[0]);
-      if (U.own1) acc[0] = fma(q.y, vv.y, acc[0]);
+      if (U.own0) acc[0] = fma(cur.C.q.x, vv.x, acc[0]);
+      if (U.own1) acc[0] = fma(cur.C.q.y, vv.y, acc[0]);
       pm = pc; pc = pn;
+    };
+    RowCA A, B;
+    if (NH_PF_CA) ld_set(A, U.Ja + 1, U.Ja);
+    for (int j = U.Ja; j < U.Jb; j += 2) {  // ping-pong operand sets: no register rotation
+      step(j, A, B);
+      if (j + 1 < U.Jb) step(j + 1, B, A);
     }
   }
   block_partials<2>(acc, P.part, buf, red);
@@ -334,7 +433,7 @@ __device__ void phase_out(const SolveP& P, bool zero) {
     }
 }
 
-__global__ void __launch_bounds__(NT, 2) k_bicgstab(SolveP P) {
+__global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
   cg::grid_group grid = cg::this_grid();
   __shared__ double red[MAXDOT][NW];
   __shared__ double bc[MAXDOT];
