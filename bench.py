@@ -37,7 +37,8 @@ UNIT = "cell-updates/s"
 # Algorithmic bytes of the dominant kernel:
 # one Jacobi-preconditioned BiCGStab iteration moves >= 20 doubles per node.
 BYTES_PER_NODE_ITER = 160.0
-ORACLE_CROP = 320          # cpu_baseline / reference sample: crop of the config-5 basin (cells per side)
+ORACLE_CROP = 640          # cpu_baseline / reference sample: crop of the config-5 basin (cells per side)
+ORACLE_STEPS = 3           # cpu_baseline leg: full RK2 steps timed on that crop (~10-30 s of host work)
 
 
 def _peaks():
@@ -102,11 +103,13 @@ class ClockSampler:
         return out
 
 
-def _oracle_sample(steps, warmup, crop=ORACLE_CROP):
+def _oracle_sample(steps, warmup, crop=None):
     """Time the CPU oracle (as it stands) on a crop of the config-5 basin: same dx, depths,
     conditioning (h/dx = 40); `steps` full RK2 NH steps after `warmup`."""
     from oracle import nh_oracle
     from paper_1706_04551_b200 import inputs
+    if crop is None:   # NH_BENCH_ORACLE_CROP: smaller sample for the CPU test-suite only
+        crop = int(os.environ.get("NH_BENCH_ORACLE_CROP", ORACLE_CROP))
     cfg = inputs.make_config(5, nx=crop, ny=crop)
     o = nh_oracle.Oracle(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["H"], **cfg["params"])
     o.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
@@ -121,6 +124,23 @@ def _oracle_sample(steps, warmup, crop=ORACLE_CROP):
                 iters_per_solve=info.iters_total / max(info.solves, 1),
                 sample=f"config 5 'source' crop {crop}x{crop} cells (same dx, depth, h/dx=40), "
                        f"{steps} full RK2 step(s) after {warmup} warm-up")
+
+
+def max_over_ranks(x, world, device=None):
+    """MAX over the ranks of a process group (any backend; world 1: identity)."""
+    if world <= 1:
+        return float(x)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(cells_per_replica, steps, world, seconds_max):
+    """Replicas only: every rank advances its own copy of the workload, so the job
+    updates world * cells * steps cells in the max-over-ranks time."""
+    return world * cells_per_replica * steps / seconds_max
 
 
 def run_reference(args):
@@ -198,11 +218,8 @@ def run_b200(args):
     sim.profile(False)
     i1 = sim.info()
     launches = sim.launch_count() - l0
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
-    value = world * nc * args.steps / (ms_max * 1e-3)
+    ms_max = max_over_ranks(ms, world, dev)
+    value = whole_job_value(nc, args.steps, world, ms_max * 1e-3)
     iters = i1.iters_total - i0.iters_total
     solves = i1.solves - i0.solves
 
@@ -251,10 +268,8 @@ def run_b200(args):
         hb.reverse()
     barrier()
     e2e_s = time.perf_counter() - t0
-    t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_value = world * nc * args.steps / float(t.item())
+    e2e_max = max_over_ranks(e2e_s, world, dev)
+    e2e_value = whole_job_value(nc, args.steps, world, e2e_max)
     st2 = sim.sync()
     io_bytes = 8 * (3 * nc + 2 * nn)
 
@@ -271,12 +286,12 @@ def run_b200(args):
                    "status": [int(st), int(st2)], "clamps": int(i1.clamps)},
         "clocks": clk,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes,
-                "d2h_bytes_per_step": io_bytes, "ms_per_step": 1e3 * float(t.item()) / args.steps},
+                "d2h_bytes_per_step": io_bytes, "ms_per_step": 1e3 * e2e_max / args.steps},
         "gpu_launches": int(launches),
         "roofline": roofline,
     }
     if rank == 0 and world == 1 and not args.no_cpu:
-        r = _oracle_sample(1, 0)
+        r = _oracle_sample(ORACLE_STEPS, 0)
         line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
                                 "sample": r["sample"], "seconds": r["seconds"]}
     if rank == 0:

@@ -53,7 +53,7 @@ bool dalloc(nh_ctx* c, T** p, size_t count) {
 }
 
 // internal node plane (ghost ring, nh_internal.cuh): the handed-out pointer addresses node (0,0)
-inline size_t node_origin(const nh_ctx* c) { return (size_t)NH_ROW_PAD * c->g.np + 2; }
+inline size_t node_origin(const nh_ctx* c) { return (size_t)NH_ROW_PAD * c->g.np + NH_COL_PAD; }
 bool nalloc(nh_ctx* c, double** p) {
   double* base = nullptr;
   if (!dalloc(c, &base, c->nni)) { *p = nullptr; return false; }

@@ -21,8 +21,9 @@
 // iteration i+1.  s is never stored.  r, p, v are double-buffered (a pass reads the old planes
 // with their halo and writes the new ones).
 //
-// Sweep geometry ("marching warps").  Node planes are stored with a ghost ring (2 columns left,
-// >= 2 right, 1+ rows above and below; pitch NP even, so every row pair is 16-byte aligned) whose
+// Sweep geometry ("marching warps").  Node planes are stored with a ghost ring (4 columns left,
+// >= 2 right, 2 rows above and below; pitch NP a multiple of 16, so every strip starts on a 32-byte
+// sector and every row on a 128-byte line, nh_internal.cuh) whose
 // distance-1 ghosts hold the mirrored / wrapped images of the boundary nodes (R10); the writer of
 // a boundary node stores its images, so no pass ever maps an index.  A warp owns a strip of 60
 // columns and marches down a band of R rows: lane l holds columns 60 s - 2 + 2 l and the next one
@@ -44,13 +45,7 @@ namespace cg = cooperative_groups;
 
 namespace {
 
-#ifndef NH_NT
-#define NH_NT 256
-#endif
-#ifndef NH_MINB
-#define NH_MINB 2
-#endif
-constexpr int NT = NH_NT, NW = NT / 32;  // CTA size, warps per CTA
+constexpr int NT = 256, NW = NT / 32;  // CTA size, warps per CTA
 constexpr int SW = 60;                 // owned columns per warp strip
 constexpr int MAXDOT = 5;
 
@@ -166,25 +161,8 @@ __device__ __forceinline__ Unit make_unit(const SolveP& P, int u, int lane) {
 }
 
 // 16-byte load of the lane's column pair of row j
-#ifndef NH_LD
-#define NH_LD 0
-#endif
 __device__ __forceinline__ double2 ld2(const double* a, const NhGrid& G, int c0, int j) {
-#if NH_LD == 1
-  return __ldcg(reinterpret_cast<const double2*>(a + nidx(G, c0, j)));
-#elif NH_LD == 2
-  return __ldcs(reinterpret_cast<const double2*>(a + nidx(G, c0, j)));
-#else
   return *reinterpret_cast<const double2*>(a + nidx(G, c0, j));
-#endif
-}
-// planes that no pass of the kernel writes (the column-scaled off-diagonals)
-__device__ __forceinline__ double2 ld2c(const double* a, const NhGrid& G, int c0, int j) {
-#if NH_LDC == 1
-  return __ldg(reinterpret_cast<const double2*>(a + nidx(G, c0, j)));
-#else
-  return ld2(a, G, c0, j);
-#endif
 }
 
 // store the lane's pair of row j (owned columns only), with ghost images on boundary nodes
@@ -211,8 +189,8 @@ struct RowC {  // coefficient row j of (A M^-1) and the shadow residual
 __device__ __forceinline__ RowC ld_rowc(const SolveP& P, int c0, int j) {
   RowC C;
   C.q = ld2(P.r0, P.G, c0, j);
-  C.e = ld2c(P.cE, P.G, c0, j); C.w = ld2c(P.cW, P.G, c0, j);
-  C.n = ld2c(P.cN, P.G, c0, j); C.s = ld2c(P.cS, P.G, c0, j);
+  C.e = ld2(P.cE, P.G, c0, j); C.w = ld2(P.cW, P.G, c0, j);
+  C.n = ld2(P.cN, P.G, c0, j); C.s = ld2(P.cS, P.G, c0, j);
   return C;
 }
 
@@ -226,17 +204,12 @@ __device__ __forceinline__ double2 stencil2(const RowC& C, double2 m, double2 c,
   return o;
 }
 
-#if defined(NH_NOINLINE)
-#define NH_PASS_INLINE __noinline__
-#else
-#define NH_PASS_INLINE __forceinline__
-#endif
-#ifndef NH_PF_B
-#define NH_PF_B 1
-#endif
-#ifndef NH_PF_CA
-#define NH_PF_CA 0
-#endif
+// Operand requests per sweep step (measured on config 5, 8192 x 8192, us per iteration: old
+// load-at-use order 2297; B prefetched + CA grouped 2069; both prefetched 2447 (CA's second operand
+// set spills); both passes out of line 2611 (the parameter block then lives in local memory);
+// cp.async rings in shared memory, 2 or 3 rows deep, 2362 / 2443).
+constexpr bool PF_B = true;    // pass B: request the next step's operands before computing this one
+constexpr bool PF_CA = false;  // pass CA: all ten operand loads of a step up front, then compute
 
 // pass B: s = r - alpha v (rows Ja-1..Jb), t = (A M^-1) s (rows Ja..Jb-1);
 // partials: t.s, t.t, s.s, r0.s, r0.t
@@ -250,7 +223,7 @@ __device__ __forceinline__ void ld_rowb(RowB& X, const SolveP& P, const double* 
   X.C = ld_rowc(P, c0, jc);
 }
 
-__device__ NH_PASS_INLINE void pass_B(const SolveP& P, double alpha, const double* r, const double* v,
+__device__ __forceinline__ void pass_B(const SolveP& P, double alpha, const double* r, const double* v,
                                     int buf, double (*red)[NW]) {
   const NhGrid& G = P.G;
   const int lane = threadIdx.x & 31;
@@ -267,7 +240,7 @@ __device__ NH_PASS_INLINE void pass_B(const SolveP& P, double alpha, const doubl
     // one sweep step: row j from the operand set `cur`; the set of the next step is requested
     // first (`nxt`; row indices clamped, the last request is never used)
     auto step = [&](int j, RowB& cur, RowB& nxt) {
-      if (NH_PF_B) ld_rowb(nxt, P, r, v, U.c0, min(j + 2, U.Jb), min(j + 1, U.Jb - 1));
+      if (PF_B) ld_rowb(nxt, P, r, v, U.c0, min(j + 2, U.Jb), min(j + 1, U.Jb - 1));
       else ld_rowb(cur, P, r, v, U.c0, j + 1, j);
       double2 sn = srow(cur.r, cur.v);
       double2 t = stencil2(cur.C, sm, sc, sn);
@@ -284,7 +257,7 @@ __device__ NH_PASS_INLINE void pass_B(const SolveP& P, double alpha, const doubl
       sm = sc; sc = sn;
     };
     RowB A, B;
-    if (NH_PF_B) ld_rowb(A, P, r, v, U.c0, U.Ja + 1, U.Ja);
+    if (PF_B) ld_rowb(A, P, r, v, U.c0, U.Ja + 1, U.Ja);
     for (int j = U.Ja; j < U.Jb; j += 2) {  // ping-pong operand sets: no register rotation
       step(j, A, B);
       if (j + 1 < U.Jb) step(j + 1, B, A);
@@ -313,7 +286,7 @@ struct RowCA {  // operands of one sweep step of pass CA: vectors of row j+1, co
 };
 
 template <bool FIRST>
-__device__ NH_PASS_INLINE void pass_CA(const SolveP& P, double alpha, double omega, double beta,
+__device__ __forceinline__ void pass_CA(const SolveP& P, double alpha, double omega, double beta,
                                      const double* r, const double* p, const double* v, double* rN,
                                      double* pN, double* vN, int buf, double (*red)[NW]) {
   const int lane = threadIdx.x & 31;
@@ -361,7 +334,7 @@ __device__ NH_PASS_INLINE void pass_CA(const SolveP& P, double alpha, double ome
       X.C = ld_rowc(P, U.c0, jc);
     };
     auto step = [&](int j, RowCA& cur, RowCA& nxt) {
-      if (NH_PF_CA) ld_set(nxt, min(j + 2, U.Jb), min(j + 1, U.Jb - 1));
+      if (PF_CA) ld_set(nxt, min(j + 2, U.Jb), min(j + 1, U.Jb - 1));
       else ld_set(cur, j + 1, j);
       double2 pn = prow(cur.V, j + 1, j + 1 < U.Jb);
       double2 vv = stencil2(cur.C, pm, pc, pn);
@@ -371,7 +344,7 @@ __device__ NH_PASS_INLINE void pass_CA(const SolveP& P, double alpha, double ome
       pm = pc; pc = pn;
     };
     RowCA A, B;
-    if (NH_PF_CA) ld_set(A, U.Ja + 1, U.Ja);
+    if (PF_CA) ld_set(A, U.Ja + 1, U.Ja);
     for (int j = U.Ja; j < U.Jb; j += 2) {  // ping-pong operand sets: no register rotation
       step(j, A, B);
       if (j + 1 < U.Jb) step(j + 1, B, A);
@@ -433,7 +406,7 @@ __device__ void phase_out(const SolveP& P, bool zero) {
     }
 }
 
-__global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
+__global__ void __launch_bounds__(NT, 2) k_bicgstab(SolveP P) {
   cg::grid_group grid = cg::this_grid();
   __shared__ double red[MAXDOT][NW];
   __shared__ double bc[MAXDOT];

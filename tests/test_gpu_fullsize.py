@@ -83,7 +83,12 @@ def test_config5_full_size_local_kernels_on_windows_and_solver_residual(O, G):
 
     n = 96
     src = (int(0.305 * nx) - n // 2, ny // 2 - n // 2)                 # the uplift
-    shore = [(nx - n, int(f * ny)) for f in (0.2, 0.7)]                # emerged coast, wet/dry
+    shore = []                                                         # shoreline (wet/dry) windows
+    for f in (0.2, 0.7):
+        j = int(f * ny)
+        ish = int(np.argmax(cfg["H"][j] <= 0.0))                       # first emerged cell of row j
+        assert 0 < ish < nx
+        shore.append((min(ish - n // 2, nx - n), j - n // 2))
     wins = _windows(nx, ny, n, seed=55, extra=[src] + shore)
 
     # --- local kernels of the pressure step on the state s0: coefficients, rhs, operator apply
