@@ -38,7 +38,7 @@ UNIT = "cell-updates/s"
 # one Jacobi-preconditioned BiCGStab iteration moves >= 20 doubles per node.
 BYTES_PER_NODE_ITER = 160.0
 ORACLE_CROP = 640          # cpu_baseline / reference sample: crop of the config-5 basin (cells per side)
-ORACLE_STEPS = 3           # cpu_baseline leg: full RK2 steps timed on that crop (~10-30 s of host work)
+ORACLE_STEPS = 5           # cpu_baseline leg: full RK2 steps timed on that crop (~10-30 s of host work)
 
 
 def _peaks():
