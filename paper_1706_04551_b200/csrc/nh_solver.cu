@@ -207,7 +207,9 @@ __device__ __forceinline__ double2 stencil2(const RowC& C, double2 m, double2 c,
 // Operand requests per sweep step (measured on config 5, 8192 x 8192, us per iteration: old
 // load-at-use order 2297; B prefetched + CA grouped 2069; both prefetched 2447 (CA's second operand
 // set spills); both passes out of line 2611 (the parameter block then lives in local memory);
-// cp.async rings in shared memory, 2 or 3 rows deep, 2362 / 2443).
+// cp.async rings in shared memory, 2 or 3 rows deep, 2362 / 2443; t recomputed in pass CA instead
+// of stored by pass B and read back, 20 instead of 22 doubles per node-iteration, 2165 (its extra
+// live rows spill at 128 registers; 2271 with 192-thread CTAs and 168 registers)).
 constexpr bool PF_B = true;    // pass B: request the next step's operands before computing this one
 constexpr bool PF_CA = false;  // pass CA: all ten operand loads of a step up front, then compute
 
