@@ -261,6 +261,16 @@ static void predictor(nho_ctx* c, const double* h, const double* qx, const doubl
       double qyn = qy[k] - lx * dU[0][2] - ly * dU[1][1];
       if (hn < 0.0) { hn = 0.0; clamps++; }                 /* R7 */
       if (hn <= c->prm.eps_dry) { qxn = 0.0; qyn = 0.0; }   /* R7 */
+      else if (c->prm.manning_n > 0.0) {
+        /* Manning friction tau = g h u n^2 |u| / h^(4/3) (L61-65, L773-775), "discretized
+         * semi-implicitly" (L249, L484; reading R27): q <- q / (1 + dt g n^2 |u*| / h*^(4/3))
+         * with the desingularised velocities of U* (S0); wet cells only. */
+        double uu = nho_dsg(hn, qxn, c->prm.delta), vv = nho_dsg(hn, qyn, c->prm.delta);
+        double speed = sqrt(uu * uu + vv * vv);
+        double h43 = hn * cbrt(hn);
+        double den = 1.0 + dt * g * c->prm.manning_n * c->prm.manning_n * speed / h43;
+        qxn = qxn / den; qyn = qyn / den;
+      }
       c->h1[k] = hn; c->qx1[k] = qxn; c->qy1[k] = qyn;
     }
   c->info.clamps += clamps;
@@ -740,6 +750,7 @@ int nho_create(nho_ctx** out, int nx, int ny, double dx, double dy, const double
   if (prm->time_order != 1 && prm->time_order != 2) return NHO_EINVAL;
   if (prm->space_order != 1 && prm->space_order != 2) return NHO_EINVAL;
   if (prm->precision != 64) return NHO_EINVAL;
+  if (!(prm->manning_n >= 0.0)) return NHO_EINVAL;
   if (prm->breaking && !(prm->B1 > 0.0 && prm->B2 > 0.0)) return NHO_EINVAL;
   if (prm->gen_on && !(prm->gen_A > 0.0 && prm->gen_h0 > 0.0 && prm->gen_Lrel > 0.0)) return NHO_EINVAL;
   size_t nc = (size_t)nx * (size_t)ny, nn = (size_t)(nx + 1) * (size_t)(ny + 1);

@@ -34,6 +34,7 @@ typedef struct {
   double B1, B2;       /* breaking onset / termination coefficients (L141-143, L635)    */
   double solver_rtol;  /* stop at ||r||_2 <= rtol*||b||_2 (reading R14), 1e-12          */
   double gen_A, gen_h0, gen_x0, gen_Lrel; /* solitary-wave generating zone at x-lo (L417-431, R18) */
+  double manning_n;    /* Gauckler-Manning coefficient n (L61-65, L773-775); 0 = frictionless     */
   int breaking;        /* 1: eddy-viscosity breaking sources on (section 3)             */
   int nonhydro;        /* 0: hydrostatic SWE path only (p = 0, w frozen)                */
   int time_order;      /* 1 or 2 (TVD RK2, L406, L516)                                  */

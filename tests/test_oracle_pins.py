@@ -554,3 +554,93 @@ def test_breaking_dissipates_on_steep_front_only(O):
             else:
                 for key in st[0]:
                     assert np.array_equal(st[0][key], st[1][key]), key
+
+
+# ---------------------------------------------------------------- Manning friction (R27)
+# tau = g h u n^2 |u| / h^(4/3), "discretized semi-implicitly" (L249):
+# q <- q / (1 + dt g n^2 |u| / h^(4/3)) after the finite-volume update.  For a uniform current over
+# a flat bottom every flux difference vanishes and the momentum equation is the ODE
+# du/dt = -k u |u|, k = g n^2 / h^(4/3), whose solution is |u|(t) = |u0| / (1 + k |u0| t); the
+# semi-implicit Euler step reproduces it exactly (1/|u| grows by k dt per step), whatever dt.
+def _uniform_current(O, nx, ny, qx0, qy0, n, **over):
+    h0 = 2.0
+    H = np.full((ny, nx), h0)
+    prm = dict(bc_xlo=O.BC_PERIODIC, bc_xhi=O.BC_PERIODIC, bc_ylo=O.BC_PERIODIC, bc_yhi=O.BC_PERIODIC,
+               manning_n=n)
+    prm.update(over)
+    o = O.Oracle(nx, ny, 0.5, 0.5, H, **prm)
+    o.set_state(H.copy(), np.full((ny, nx), qx0), np.full((ny, nx), qy0))
+    return o, h0
+
+
+@pytest.mark.parametrize("nonhydro", [0, 1])
+def test_manning_uniform_current_decays_by_the_closed_form(O, nonhydro):
+    n, g = 0.1, 9.81
+    o, h0 = _uniform_current(O, 16, 12, 3.0, -4.0, n, time_order=1, nonhydro=nonhydro)
+    o.step(100)
+    s, T = o.get_state(), o.info().t
+    k = g * n * n / h0 ** (4.0 / 3.0)
+    sp0 = 5.0 / h0
+    sp = sp0 / (1.0 + k * sp0 * T)
+    assert T > 0.5 and sp < 0.98 * sp0                      # friction has acted
+    assert np.max(np.abs(s["h"] - h0)) == 0.0                # friction never touches h (mass)
+    assert np.max(np.abs(s["qx"] - h0 * sp * 0.6)) <= 1e-13
+    assert np.max(np.abs(s["qy"] + h0 * sp * 0.8)) <= 1e-13  # direction preserved
+    assert np.max(np.abs(s["p"])) <= 1e-12 and np.max(np.abs(s["w"])) <= 1e-12
+
+
+def test_manning_rk2_converges_to_the_decay_law(O):
+    # Each stage applies the exact flow of the friction ODE, so the TVD-RK2 average
+    # (U^n + Phi(Phi(U^n))) / 2 = (u(t) + u(t + 2 dt)) / 2 differs from u(t + dt) by dt^2 u''/2 per
+    # step: with the semi-implicit treatment the friction term is first-order accurate in time
+    # (the paper claims second order for the flux and non-hydrostatic terms only, L249).
+    n, g = 0.1, 9.81
+    errs = []
+    for cfl in (0.8, 0.4):
+        o, h0 = _uniform_current(O, 8, 8, 5.0, 0.0, n, time_order=2, nonhydro=0, cfl=cfl)
+        steps = 0
+        while o.info().t < 1.0:
+            o.step(1)
+            steps += 1
+        k = g * n * n / h0 ** (4.0 / 3.0)
+        u0 = 5.0 / h0
+        exact = h0 * u0 / (1.0 + k * u0 * o.info().t)
+        errs.append(abs(o.get_state()["qx"][0, 0] - exact))
+    assert 0.0 < errs[1] < errs[0] < 2e-3 and 1.7 < errs[0] / errs[1] < 2.3   # dt halves: error / 2
+
+
+def test_manning_zero_is_bit_identical_and_rest_stays_at_rest(O):
+    cfg = inputs.make_config(2, nx=64, ny=64)
+    a = make(O, cfg)
+    b = make(O, cfg, manning_n=0.0)
+    c = make(O, cfg, manning_n=0.025)
+    for o in (a, b, c):
+        o.step(5)
+    sa, sb, sc = a.get_state(), b.get_state(), c.get_state()
+    for k in sa:
+        assert np.array_equal(sa[k], sb[k])
+    assert np.max(np.abs(sc["qx"])) == 0.0 and np.max(np.abs(sc["qy"])) == 0.0
+    assert np.max(np.abs(sc["h"] - cfg["h"])) <= 1e-13 * 5.0
+
+
+def test_manning_conserves_mass_and_dissipates_energy(O):
+    s = inputs.random_smooth_state(48, 40, 0.5, 0.5, seed=5, depth=1.0, dry_fraction=0.0)
+    bc = dict(bc_xlo=O.BC_WALL, bc_xhi=O.BC_WALL, bc_ylo=O.BC_PERIODIC, bc_yhi=O.BC_PERIODIC)
+    out = {}
+    for n in (0.0, 0.05):
+        o = O.Oracle(48, 40, 0.5, 0.5, s["H"], manning_n=n, **bc)
+        o.set_state(s["h"], s["qx"], s["qy"], s["w"], s["p"])
+        o.step(30)
+        assert o.info().clamps == 0
+        out[n] = o.get_state()
+    m0 = np.sum(s["h"])
+    assert abs(np.sum(out[0.05]["h"]) - m0) <= 1e-12 * m0
+
+    def kinetic(st):
+        return np.sum((st["qx"] ** 2 + st["qy"] ** 2) / st["h"])
+    assert kinetic(out[0.05]) < 0.995 * kinetic(out[0.0])          # 30 short steps at n = 0.05: ~1 %
+
+
+def test_manning_negative_coefficient_is_rejected(O):
+    with pytest.raises(O.OracleError):
+        O.Oracle(8, 8, 1.0, 1.0, np.ones((8, 8)), manning_n=-0.01)
