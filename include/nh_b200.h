@@ -58,6 +58,7 @@ typedef struct {
   double B1, B2;      /* breaking onset / termination coefficients, 0.15 / 0.5 (L141-143, L635) */
   double solver_rtol; /* BiCGStab stops at ||r||_2 <= rtol ||b||_2, default 1e-12 (R14)     */
   double gen_A, gen_h0, gen_x0, gen_Lrel; /* solitary-wave generating zone at x-lo (L417-431, R18) */
+  double manning_n;   /* Gauckler-Manning n (L61-65, L773-775), semi-implicit (R27); default 0 = off */
   int breaking;       /* 1: eddy-viscosity breaking sources on (section 3, eqs (8)-(12))    */
   int nonhydro;       /* 0: hydrostatic SWE path only (p = 0, w frozen); default 1          */
   int time_order;     /* 1, or 2 = two-stage TVD Runge-Kutta (L406, L516, L544); default 2  */

@@ -225,6 +225,7 @@ int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* 
   if (prm->time_order != 1 && prm->time_order != 2) return NH_EINVAL;
   if (prm->space_order != 1 && prm->space_order != 2) return NH_EINVAL;
   if (prm->precision != 64) return NH_EINVAL;
+  if (!(prm->manning_n >= 0.0)) return NH_EINVAL;
   if (prm->breaking && !(prm->B1 > 0.0 && prm->B2 > 0.0)) return NH_EINVAL;
   if (prm->gen_on && !(prm->gen_A > 0.0 && prm->gen_h0 > 0.0 && prm->gen_Lrel > 0.0)) return NH_EINVAL;
 

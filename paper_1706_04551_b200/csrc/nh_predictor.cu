@@ -97,7 +97,8 @@ __device__ __forceinline__ void face_fluct(double g, double hm, double etam, dou
 }
 
 __global__ void __launch_bounds__(PTX* PTY)
-k_predictor(NhGrid G, double g, double delta, double eps_dry, int order, const NhScal* sc,
+k_predictor(NhGrid G, double g, double delta, double eps_dry, double manning_n, int order,
+            const NhScal* sc,
             const double* __restrict__ H, const double* __restrict__ h,
             const double* __restrict__ qx, const double* __restrict__ qy,
             double* __restrict__ h1, double* __restrict__ qx1, double* __restrict__ qy1,
@@ -169,6 +170,15 @@ k_predictor(NhGrid G, double g, double delta, double eps_dry, int order, const N
   double qyn = qy[k] - lxr * dU[0][2] - lyr * dU[1][1];
   if (hn < 0.0) { hn = 0.0; atomicAdd(clamps, 1ULL); }  // R7
   if (hn <= eps_dry) { qxn = 0.0; qyn = 0.0; }          // R7
+  else if (manning_n > 0.0) {
+    // Manning friction tau = g h u n^2 |u| / h^(4/3) (L61-65, L773-775), semi-implicit (L249, R27):
+    // q <- q / (1 + dt g n^2 |u*| / h*^(4/3)), desingularised velocities of U*, wet cells only
+    double uu = nh_dsg(hn, qxn, delta), vv = nh_dsg(hn, qyn, delta);
+    double speed = sqrt(uu * uu + vv * vv);
+    double h43 = hn * cbrt(hn);
+    double den = 1.0 + dt * g * manning_n * manning_n * speed / h43;
+    qxn = qxn / den; qyn = qyn / den;
+  }
   h1[k] = hn; qx1[k] = qxn; qy1[k] = qyn;
 }
 
@@ -285,7 +295,7 @@ void nh_launch_predictor(nh_ctx* c, const double* h, const double* qx, const dou
                          double* qx1, double* qy1) {
   dim3 grid((c->g.nx + PTX - 1) / PTX, (c->g.ny + PTY - 1) / PTY), block(PTX, PTY);
   k_predictor<<<grid, block, 0, c->stream>>>(c->g, c->prm.g, c->prm.delta, c->prm.eps_dry,
-                                             c->prm.space_order, c->sc, c->H, h, qx, qy, h1, qx1,
+                                             c->prm.manning_n, c->prm.space_order, c->sc, c->H, h, qx, qy, h1, qx1,
                                              qy1, (unsigned long long*)&c->sc->clamps);
   c->launches++;
 }

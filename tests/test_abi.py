@@ -46,7 +46,7 @@ def test_struct_layouts_match_the_header():
 #include <stddef.h>
 #include "nh_b200.h"
 int main(void) {
-  printf("%zu %zu %zu %zu %zu %zu %zu\n", sizeof(nh_params), offsetof(nh_params, gen_Lrel),
+  printf("%zu %zu %zu %zu %zu %zu %zu\n", sizeof(nh_params), offsetof(nh_params, manning_n),
          offsetof(nh_params, breaking), offsetof(nh_params, solver_maxit), offsetof(nh_params, precision),
          sizeof(nh_info), offsetof(nh_info, iters_last));
   return 0;
@@ -61,7 +61,7 @@ int main(void) {
         out = subprocess.run([exe], check=True, capture_output=True, text=True).stdout.split()
     got = [int(x) for x in out]
     P, I = nh.Params, nh.Info
-    want = [C.sizeof(P), P.gen_Lrel.offset, P.breaking.offset, P.solver_maxit.offset,
+    want = [C.sizeof(P), P.manning_n.offset, P.breaking.offset, P.solver_maxit.offset,
             P.precision.offset, C.sizeof(I), I.iters_last.offset]
     assert got == want
 

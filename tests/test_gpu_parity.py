@@ -335,3 +335,60 @@ def test_get_state_roundtrip_periodic_node_lines(G):
     assert np.array_equal(s["h"], cfg["h"]) and np.array_equal(s["qx"], cfg["qx"])
     assert np.array_equal(s["w"][:-1, :-1], cfg["w"][:-1, :-1])
     assert np.array_equal(s["w"][-1, :], s["w"][0, :]) and np.array_equal(s["p"][:, -1], s["p"][:, 0])
+
+
+# ---------------------------------------------------------------- Manning friction (R27)
+# cbrt() is not correctly rounded on either side, so the friction factor may differ in the last
+# place: these comparisons use the north_star tolerances instead of bit equality.
+@pytest.mark.parametrize("bcs", [BCS[1], BCS[2]])
+@pytest.mark.parametrize("dry", [0.0, 0.3])
+def test_manning_predictor_and_steps_parity(O, G, bcs, dry):
+    cfg = rnd_cfg(70, 45, bcs, seed=71, dry=dry, manning_n=0.03, breaking=1, B1=0.02, B2=0.05)
+    o, g = both(O, G, cfg)
+    o.hydrostatic_step(0.0)
+    g.hydrostatic_step(0.0)
+    assert g.sync() == 0
+    so, sg = o.get_state(), g.get_state()
+    assert np.array_equal(so["h"], sg["h"])                    # friction never touches h
+    for k in ("qx", "qy"):
+        assert np.max(np.abs(so[k] - sg[k])) <= 1e-14 * max(np.max(np.abs(so[k])), 1.0)
+    assert o.info().clamps == g.info().clamps
+    o.step(4)
+    g.step(4)
+    assert g.sync() == 0
+    assert_parity(g.get_state(), o.get_state(), cfg["H"], cfg["h0"])
+
+
+def test_manning_uniform_current_closed_form_on_gpu(G):
+    # the decay law |u|(t) = |u0| / (1 + k |u0| t), k = g n^2 / h^(4/3) (see test_oracle_pins.py)
+    nx, ny, h0, n, grav = 96, 40, 2.0, 0.1, 9.81
+    H = np.full((ny, nx), h0)
+    g = G.NH(nx, ny, 0.5, 0.5, H, bc_xlo=PER, bc_xhi=PER, bc_ylo=PER, bc_yhi=PER, manning_n=n,
+             time_order=1)
+    g.set_state(H.copy(), np.full((ny, nx), 3.0), np.full((ny, nx), -4.0))
+    g.step(100)
+    assert g.sync() == 0
+    s, T = g.get_state(), g.info().t
+    k = grav * n * n / h0 ** (4.0 / 3.0)
+    sp = 2.5 / (1.0 + k * 2.5 * T)
+    assert sp < 0.9 * 2.5
+    assert np.max(np.abs(s["qx"] - h0 * sp * 0.6)) <= 1e-13
+    assert np.max(np.abs(s["qy"] + h0 * sp * 0.8)) <= 1e-13
+    assert np.max(np.abs(s["h"] - h0)) == 0.0
+
+
+def test_manning_beach_reduced_parity(O, G):
+    # config 4 with the paper's run-up roughness n = 0.01 (L631), reduced size
+    cfg = inputs.make_config(4, nx=512, ny=8)
+    o, g = both(O, G, cfg, manning_n=0.01)
+    for _ in range(2):
+        o.step(75)
+        g.step(75)
+        assert g.sync() == 0
+        assert_parity(g.get_state(), o.get_state(), cfg["H"], cfg["h0"])
+
+
+def test_manning_negative_coefficient_is_rejected(G):
+    with pytest.raises(G.NHError) as e:
+        G.NH(8, 8, 1.0, 1.0, np.ones((8, 8)), manning_n=-1.0)
+    assert e.value.code == G.EINVAL
