@@ -536,6 +536,113 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
 
 /* ------------------------------------------------------------------------------------ */
 /* S6: breaking sources (section 3, eqs (9)-(12); 2D reading R12, node reading R13).        */
+/* S9' (solver = 1): the paper's solver, "an iterative Jacobi method combined with a scheduled
+ * relaxation method following [2]" with the stopping rule (32).
+ * The paper prints neither the relaxation factors nor the cycle; reading R28:
+ *   - row-scaled system: dinv = 1/A_C, c_X = A_X dinv, b' = b dinv (Jacobi's D^-1);
+ *   - rho = max_n ((|c_E|+|c_W|)+|c_N|)+|c_S| < 1 is the Gershgorin radius of D^-1 A about 1
+ *     (strict diagonal dominance, L503-505), so the spectrum lies in [1-rho, 1+rho];
+ *   - one relaxation cycle has M factors, the reciprocals of the Chebyshev nodes of that interval,
+ *       omega_k = 1 / (1 - rho cos(pi (2k-1) / (2M))),  k = 1..M
+ *     (the optimal scheduled-relaxation factors are exactly these: Adsuara et al.'s follow-up to
+ *     [2]), applied in the Lebedev-Finogenov order for powers of two (perm_1 = (1); perm_2m =
+ *     (p_1, 2m+1-p_1, p_2, 2m+1-p_2, ...)), which keeps round-off bounded for long cycles;
+ *   - M = smallest power of two with M sqrt(2 (1-rho)) >= 7.6 (one cycle then damps every mode
+ *     about 1000-fold), at most srj_mmax;
+ *   - iteration k: z = b' - (x + c_E x_E + c_W x_W + c_N x_N + c_S x_S) is the increment of the
+ *     plain Jacobi method; stop if E = ||z||_inf < srj_eps, eq. (32) (x is then the answer);
+ *     otherwise x <- x + omega z.  No dot products; every node update depends on x of the
+ *     previous sweep only, so the result does not depend on the sweep order.
+ * x: start -> solution.  res_out = the last E. */
+static int srj_solve(nho_ctx* c, const double* h, const double* z, const double* b, double* x,
+                     int* iters_out, double* res_out) {
+  const int nnx = c->nnx, nny = c->nny, maxit = c->prm.solver_maxit;
+  double *dinv = c->kdiag, *ce = c->kph, *cw = c->ksh, *cn = c->ks, *cs = c->kt, *bp = c->kr;
+  double *xn = c->kv;
+  *iters_out = 0; *res_out = 0.0;
+  double rho = 0.0, bmax = 0.0;
+  int bad = 0;
+#pragma omp parallel for if (c->ny >= 48) schedule(static) reduction(max : rho, bmax) reduction(| : bad)
+  for (int J = 0; J < nny; ++J)
+    for (int I = 0; I < nnx; ++I) {
+      double AC, AE, AW, AN, AS;
+      node_coeffs(c, h, z, I, J, &AC, &AE, &AW, &AN, &AS);
+      size_t k = NIDX(c, I, J);
+      double di = 1.0 / AC;
+      dinv[k] = di;
+      ce[k] = AE * di; cw[k] = AW * di; cn[k] = AN * di; cs[k] = AS * di;
+      bp[k] = b[k] * di;
+      double rad = ((fabs(ce[k]) + fabs(cw[k])) + fabs(cn[k])) + fabs(cs[k]);
+      if (rad > rho) rho = rad;
+      if (fabs(bp[k]) > bmax) bmax = fabs(bp[k]);
+      if (!(bp[k] == bp[k]) || isinf(bp[k])) bad = 1;
+    }
+  if (bad) return NHO_ENAN;
+  if (bmax == 0.0) {  /* same convention as the BiCGStab path: b = 0 => p~ = 0, zero iterations */
+#pragma omp parallel for if (c->ny >= 48) schedule(static)
+    for (int J = 0; J < nny; ++J)
+      for (int I = 0; I < nnx; ++I) x[NIDX(c, I, J)] = 0.0;
+    return NHO_OK;
+  }
+  if (!(rho < 1.0)) {
+    snprintf(c->err, sizeof(c->err), "srj: matrix not strictly diagonally dominant (rho = %g)", rho);
+    return NHO_ENOCONV;
+  }
+  /* cycle length and schedule */
+  const double gap = sqrt(2.0 * (1.0 - rho));
+  int M = 1;
+  while (M < c->prm.srj_mmax && (double)M * gap < 7.6) M *= 2;
+  int* perm = (int*)malloc(sizeof(int) * (size_t)M);
+  double* omega = (double*)malloc(sizeof(double) * (size_t)M);
+  if (!perm || !omega) { free(perm); free(omega); return NHO_ENOMEM; }
+  perm[0] = 1;
+  for (int m = 1; m < M; m *= 2)          /* perm_2m from perm_m, in place from the back */
+    for (int i = m - 1; i >= 0; --i) {
+      int a = perm[i];
+      perm[2 * i] = a; perm[2 * i + 1] = 2 * m + 1 - a;
+    }
+  for (int i = 0; i < M; ++i) {
+    double cosv = cos(3.14159265358979323846 * (double)(2 * perm[i] - 1) / (double)(2 * M));
+    omega[i] = 1.0 / (1.0 - rho * cosv);
+  }
+  int iters = 0, status = NHO_OK;
+  double E = 0.0;
+  for (;;) {
+    const double om = omega[iters % M];
+    double Emax = 0.0;
+    int nan = 0;
+#pragma omp parallel for if (c->ny >= 48) schedule(static) reduction(max : Emax) reduction(| : nan)
+    for (int J = 0; J < nny; ++J)
+      for (int I = 0; I < nnx; ++I) {
+        size_t k = NIDX(c, I, J);
+        double ax = x[k] + (((ce[k] * node_val(c, x, I + 1, J) + cw[k] * node_val(c, x, I - 1, J)) +
+                             cn[k] * node_val(c, x, I, J + 1)) + cs[k] * node_val(c, x, I, J - 1));
+        double zz = bp[k] - ax;
+        double az = fabs(zz);
+        if (az > Emax) Emax = az;
+        if (!(zz == zz)) nan = 1;
+        xn[k] = x[k] + om * zz;
+      }
+    E = Emax;
+    if (nan) { status = NHO_ENAN; break; }
+    if (E < c->prm.srj_eps) break;               /* eq. (32): x is the accepted iterate */
+    if (iters >= maxit) { status = NHO_ENOCONV; break; }
+#pragma omp parallel for if (c->ny >= 48) schedule(static)
+    for (int J = 0; J < nny; ++J)
+      for (int I = 0; I < nnx; ++I) x[NIDX(c, I, J)] = xn[NIDX(c, I, J)];
+    iters++;
+  }
+  free(perm); free(omega);
+  *iters_out = iters; *res_out = E;
+  return status;
+}
+
+static int solve_system(nho_ctx* c, const double* h, const double* z, const double* b, double* x,
+                        int* iters_out, double* res_out) {
+  if (c->prm.solver == 1) return srj_solve(c, h, z, b, x, iters_out, res_out);
+  return bicgstab(c, h, z, b, x, iters_out, res_out);
+}
+
 /* in: U* = (h1,qx1,qy1), w_in; out: q** = (qx2,qy2), w2.                                   */
 static void breaking_sources(nho_ctx* c, const double* w_in, double dt) {
   const double g = c->prm.g, delta = c->prm.delta, eps = c->prm.eps_dry;
@@ -696,7 +803,7 @@ static int nonhydro_part(nho_ctx* c, const double* w_in, double dt, double* qx_o
       c->b[NIDX(c, I, J)] = (dt > 0.0) ? -node_B(c, c->h1, c->qx2, c->qy2, c->z, c->w2, I, J) / dt
                                        : 0.0;   /* R26: all-dry domain, dt = 0 => p~ = 0 */
   int iters = 0; double relres = 0.0;
-  int st = bicgstab(c, c->h1, c->z, c->b, c->p, &iters, &relres);
+  int st = solve_system(c, c->h1, c->z, c->b, c->p, &iters, &relres);
   c->info.iters_last = iters;
   c->info.iters_total += iters;
   c->info.solves += 1;
@@ -733,6 +840,7 @@ void nho_default_params(nho_params* prm) {
   prm->breaking = 0; prm->nonhydro = 1; prm->time_order = 2; prm->space_order = 2;
   prm->bc_xlo = prm->bc_xhi = prm->bc_ylo = prm->bc_yhi = NHO_BC_OUTFLOW;
   prm->solver_maxit = 10000; prm->gen_on = 0; prm->precision = 64;
+  prm->solver = 0; prm->srj_eps = 1e-5; prm->srj_mmax = 256;
 }
 
 static int bc_ok(int b) { return b == NHO_BC_PERIODIC || b == NHO_BC_WALL || b == NHO_BC_OUTFLOW; }
@@ -751,6 +859,9 @@ int nho_create(nho_ctx** out, int nx, int ny, double dx, double dy, const double
   if (prm->space_order != 1 && prm->space_order != 2) return NHO_EINVAL;
   if (prm->precision != 64) return NHO_EINVAL;
   if (!(prm->manning_n >= 0.0)) return NHO_EINVAL;
+  if (prm->solver != 0 && prm->solver != 1) return NHO_EINVAL;
+  if (prm->solver == 1 && (!(prm->srj_eps > 0.0) || prm->srj_mmax < 1 || prm->srj_mmax > 4096 ||
+                           (prm->srj_mmax & (prm->srj_mmax - 1)) != 0)) return NHO_EINVAL;
   if (prm->breaking && !(prm->B1 > 0.0 && prm->B2 > 0.0)) return NHO_EINVAL;
   if (prm->gen_on && !(prm->gen_A > 0.0 && prm->gen_h0 > 0.0 && prm->gen_Lrel > 0.0)) return NHO_EINVAL;
   size_t nc = (size_t)nx * (size_t)ny, nn = (size_t)(nx + 1) * (size_t)(ny + 1);
@@ -953,7 +1064,7 @@ int nho_solve(nho_ctx* c, const double* b_nodes, double* x_nodes, int* iters, do
   nodes_in(c, b_nodes, c->b);
   nodes_in(c, x_nodes, c->w2);
   compute_z(c, c->h, c->z);
-  int st = bicgstab(c, c->h, c->z, c->b, c->w2, &it, &rr);
+  int st = solve_system(c, c->h, c->z, c->b, c->w2, &it, &rr);
   nodes_out(c, c->w2, x_nodes);
   if (iters) *iters = it;
   if (relres) *relres = rr;

@@ -35,6 +35,7 @@ typedef struct {
   double solver_rtol;  /* stop at ||r||_2 <= rtol*||b||_2 (reading R14), 1e-12          */
   double gen_A, gen_h0, gen_x0, gen_Lrel; /* solitary-wave generating zone at x-lo (L417-431, R18) */
   double manning_n;    /* Gauckler-Manning coefficient n (L61-65, L773-775); 0 = frictionless     */
+  double srj_eps;      /* solver 1: stop when the Jacobi increment of (32) is < srj_eps (L507-514) */
   int breaking;        /* 1: eddy-viscosity breaking sources on (section 3)             */
   int nonhydro;        /* 0: hydrostatic SWE path only (p = 0, w frozen)                */
   int time_order;      /* 1 or 2 (TVD RK2, L406, L516)                                  */
@@ -43,6 +44,9 @@ typedef struct {
   int solver_maxit;
   int gen_on;
   int precision;       /* 64 only in the oracle                                         */
+  int solver;          /* 0: Jacobi-preconditioned BiCGStab (R14); 1: the paper's Jacobi method
+                          with scheduled relaxation (L507-514; reading R28)                     */
+  int srj_mmax;        /* solver 1: longest relaxation cycle (power of two), default 256        */
   int reserved;
 } nho_params;
 

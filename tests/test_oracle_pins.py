@@ -644,3 +644,106 @@ def test_manning_conserves_mass_and_dissipates_energy(O):
 def test_manning_negative_coefficient_is_rejected(O):
     with pytest.raises(O.OracleError):
         O.Oracle(8, 8, 1.0, 1.0, np.ones((8, 8)), manning_n=-0.01)
+
+
+# ---------------------------------------------------------------- solver 1: the paper's Jacobi
+# method with scheduled relaxation and the stopping rule (32) (L507-514; reading R28)
+@pytest.mark.parametrize("bx", [(PER, PER), (OUT, WALL)])
+@pytest.mark.parametrize("by", [(PER, PER), (WALL, OUT)])
+@pytest.mark.parametrize("dry", [0.0, 0.3])
+def test_srj_matches_dense_lu(O, bx, by, dry):
+    nx, ny, dx, dy = 9, 7, 0.3, 0.4
+    st = inputs.random_smooth_state(nx, ny, dx, dy, seed=2, depth=1.0, rough=0.4, dry_fraction=dry)
+    o = O.Oracle(nx, ny, dx, dy, st["H"], bc_xlo=bx[0], bc_xhi=bx[1], bc_ylo=by[0], bc_yhi=by[1],
+                 solver=1, srj_eps=1e-14)
+    o.set_state(st["h"], st["qx"], st["qy"], st["w"])
+    A, nnx, nny = dense_A(o, ny, nx, bx[0] == PER, by[0] == PER)
+    b = o.rhs(0.01)
+    x_ref = np.linalg.solve(A, b[:nny, :nnx].ravel()).reshape(nny, nnx)
+    x, it, E = o.solve(b)
+    assert E < 1e-14 and 0 < it < 2000
+    np.testing.assert_allclose(x[:nny, :nnx], x_ref, rtol=0, atol=1e-10 * np.abs(x_ref).max())
+
+
+def test_srj_cycle_of_one_is_the_plain_jacobi_method_with_rule_32(O):
+    # srj_mmax = 1: omega = 1 / (1 - rho cos(pi/2)) = 1 to round-off: textbook Jacobi
+    # x <- x + D^-1 (b - A x), stopped by (32) on the increment.
+    nx, ny, dx, dy = 12, 10, 0.5, 0.4
+    st = inputs.random_smooth_state(nx, ny, dx, dy, seed=3, depth=0.4, rough=0.3)
+    o = O.Oracle(nx, ny, dx, dy, st["H"], bc_xlo=WALL, bc_xhi=OUT, bc_ylo=PER, bc_yhi=PER,
+                 solver=1, srj_eps=1e-9, srj_mmax=1)
+    o.set_state(st["h"], st["qx"], st["qy"], st["w"])
+    A, nnx, nny = dense_A(o, ny, nx, False, True)
+    b = o.rhs(0.02)
+    x, it, E = o.solve(b)
+    D = np.diag(A)
+    bb = b[:nny, :nnx].ravel()
+    y = np.zeros_like(bb)
+    k = 0
+    while True:
+        z = (bb - A @ y) / D
+        if np.max(np.abs(z)) < 1e-9:
+            break
+        y = y + z
+        k += 1
+    assert it == k and 5 < k < 2000
+    np.testing.assert_allclose(x[:nny, :nnx].ravel(), y, rtol=0, atol=1e-13 * np.abs(y).max())
+
+
+@pytest.mark.parametrize("hdx", [4.0, 12.0])
+def test_srj_cycle_meets_the_chebyshev_bound_on_the_flat_bottom_operator(O, hdx):
+    # Flat bottom, periodic: A = A_C I - (h^2/2dx^2)(shift sum) is symmetric with constant diagonal,
+    # the spectrum of D^-1 A lies in [1-rho, 1+rho], and after one full cycle of M Chebyshev factors
+    # the error is reduced by at least 1 / T_M(1/rho) in the 2-norm, T_M(s) = cosh(M acosh s).  A
+    # wrong factor, a wrong node formula or an incomplete permutation breaks the bound (constant
+    # omega = 1 over M sweeps only reaches rho^M).
+    n, dx = 32, 0.25
+    h0 = hdx * dx
+    H = np.full((n, n), h0)
+    rho = (2 * hdx ** 2) / (2.0 + 2 * hdx ** 2)
+    gap = np.sqrt(2.0 * (1.0 - rho))
+    M = 1
+    while M * gap < 7.6:
+        M *= 2
+    o = O.Oracle(n, n, dx, dx, H, bc_xlo=PER, bc_xhi=PER, bc_ylo=PER, bc_yhi=PER, solver=1,
+                 srj_eps=1e-300, solver_maxit=M)
+    o.set_state(H.copy(), np.zeros((n, n)), np.zeros((n, n)))
+    rng = np.random.Generator(np.random.PCG64(9))
+    xs = np.zeros((n + 1, n + 1))
+    xs[:n, :n] = rng.standard_normal((n, n))
+    xs[n, :] = xs[0, :]
+    xs[:, n] = xs[:, 0]
+    b = o.apply_A(xs)
+    x, it, E = o.solve(b, allow_noconv=True)
+    assert it == M
+    err = np.linalg.norm((x - xs)[:n, :n]) / np.linalg.norm(xs[:n, :n])
+    bound = 1.0 / np.cosh(M * np.arccosh(1.0 / rho))
+    assert err <= bound * (1.0 + 1e-6), (err, bound, M)
+    assert err >= 1e-3 * bound and bound < 2.1e-3            # and rho^M is far above the bound
+    assert rho ** M > 30.0 * bound
+
+
+def test_srj_step_agrees_with_bicgstab_step_within_the_solver_tolerances(O):
+    s = inputs.random_smooth_state(40, 32, 0.2, 0.2, seed=12, depth=1.0, dry_fraction=0.2)
+    bc = dict(bc_xlo=OUT, bc_xhi=WALL, bc_ylo=PER, bc_yhi=PER)
+    out = []
+    for kw in (dict(solver=0), dict(solver=1, srj_eps=1e-13)):
+        o = O.Oracle(40, 32, 0.2, 0.2, s["H"], **bc, **kw)
+        o.set_state(s["h"], s["qx"], s["qy"], s["w"], s["p"])
+        o.step(3)
+        assert o.info().iters_total > 0
+        out.append(o.get_state())
+    for k in ("h", "qx", "qy", "w", "p"):
+        scale = max(np.max(np.abs(out[0][k])), 1e-3)
+        assert np.max(np.abs(out[0][k] - out[1][k])) <= 1e-9 * scale, k
+
+
+def test_srj_zero_rhs_gives_zero_pressure_and_bad_parameters_are_rejected(O):
+    cfg = inputs.make_config(2, nx=48, ny=48)
+    o = make(O, cfg, solver=1)
+    o.step(3)
+    s = o.get_state()
+    assert np.all(s["p"] == 0.0) and o.info().iters_total == 0 and o.info().solves == 6
+    for bad in (dict(solver=2), dict(solver=1, srj_mmax=48), dict(solver=1, srj_eps=0.0)):
+        with pytest.raises(O.OracleError):
+            O.Oracle(8, 8, 1.0, 1.0, np.ones((8, 8)), **bad)
