@@ -59,6 +59,7 @@ typedef struct {
   double solver_rtol; /* BiCGStab stops at ||r||_2 <= rtol ||b||_2, default 1e-12 (R14)     */
   double gen_A, gen_h0, gen_x0, gen_Lrel; /* solitary-wave generating zone at x-lo (L417-431, R18) */
   double manning_n;   /* Gauckler-Manning n (L61-65, L773-775), semi-implicit (R27); default 0 = off */
+  double srj_eps;     /* solver 1: stop when the Jacobi increment of eq. (32) is < srj_eps; 1e-5  */
   int breaking;       /* 1: eddy-viscosity breaking sources on (section 3, eqs (8)-(12))    */
   int nonhydro;       /* 0: hydrostatic SWE path only (p = 0, w frozen); default 1          */
   int time_order;     /* 1, or 2 = two-stage TVD Runge-Kutta (L406, L516, L544); default 2  */
@@ -67,6 +68,11 @@ typedef struct {
   int solver_maxit;   /* default 10000                                                      */
   int gen_on;         /* 1: generating relaxation zone active                               */
   int precision;      /* 64 (fp64).  32 is not built yet: NH_EINVAL                         */
+  int solver;         /* 0 (default): Jacobi-preconditioned BiCGStab to solver_rtol (R14);
+                         1: the paper's Jacobi method with scheduled relaxation and stopping
+                         rule (32) (L507-514; R28): no dot products, results bit-identical
+                         to the CPU oracle's                                                 */
+  int srj_mmax;       /* solver 1: longest relaxation cycle, a power of two <= 4096; default 256 */
   int reserved;
 } nh_params;
 

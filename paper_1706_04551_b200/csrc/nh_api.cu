@@ -65,6 +65,7 @@ void free_all(nh_ctx* c) {
   for (void* p : c->raw) if (p) cudaFree(p);
   c->raw.clear();
   if (c->part) cudaFree(c->part);
+  if (c->srj_cos) cudaFree(c->srj_cos);
   if (c->sc_host) cudaFreeHost(c->sc_host);
   for (int k = 0; k < NH_PROF_CATS; ++k)
     for (auto& ev : c->prof_ev[k]) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
@@ -160,7 +161,8 @@ void nonhydro_part(nh_ctx* c, const double* h1, const double* qx1, const double*
     nh_launch_compute_z(c, h1, c->z);
     nh_launch_rhs(c, h1, qxs, qys, c->z, ws, c->b, 0);
     nh_launch_coeffs(c, h1, c->z);
-    nh_launch_scale_coeffs(c);
+    if (c->prm.solver == 1) nh_launch_scale_rows(c, c->b, c->kr);
+    else nh_launch_scale_coeffs(c);
   }
   {
     ProfScope ps(c, NH_PROF_SOLVER);
@@ -210,6 +212,7 @@ void nh_default_params(nh_params* prm) {
   prm->breaking = 0; prm->nonhydro = 1; prm->time_order = 2; prm->space_order = 2;
   prm->bc_xlo = prm->bc_xhi = prm->bc_ylo = prm->bc_yhi = NH_BC_OUTFLOW;
   prm->solver_maxit = 10000; prm->gen_on = 0; prm->precision = 64;
+  prm->solver = 0; prm->srj_eps = 1e-5; prm->srj_mmax = 256;
 }
 
 int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* H,
@@ -226,6 +229,9 @@ int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* 
   if (prm->space_order != 1 && prm->space_order != 2) return NH_EINVAL;
   if (prm->precision != 64) return NH_EINVAL;
   if (!(prm->manning_n >= 0.0)) return NH_EINVAL;
+  if (prm->solver != 0 && prm->solver != 1) return NH_EINVAL;
+  if (prm->solver == 1 && (!(prm->srj_eps > 0.0) || prm->srj_mmax < 1 || prm->srj_mmax > 4096 ||
+                           (prm->srj_mmax & (prm->srj_mmax - 1)) != 0)) return NH_EINVAL;
   if (prm->breaking && !(prm->B1 > 0.0 && prm->B2 > 0.0)) return NH_EINVAL;
   if (prm->gen_on && !(prm->gen_A > 0.0 && prm->gen_h0 > 0.0 && prm->gen_Lrel > 0.0)) return NH_EINVAL;
 
@@ -503,7 +509,8 @@ int nh_solve(nh_ctx* c, const double* b_nodes, double* x_nodes, int* iters, doub
   if (node_in(c, c->b, b_nodes) || node_in(c, c->w2, x_nodes)) return NH_ECUDA;
   nh_launch_compute_z(c, c->h[c->cur], c->z);
   nh_launch_coeffs(c, c->h[c->cur], c->z);
-  nh_launch_scale_coeffs(c);
+  if (c->prm.solver == 1) nh_launch_scale_rows(c, c->b, c->kr);
+  else nh_launch_scale_coeffs(c);
   nh_launch_solve(c, c->b, c->w2, 0);
   if (node_out(c, c->w2, x_nodes)) return NH_ECUDA;
   if (check_launch(c) != NH_OK) return NH_ECUDA;

@@ -36,6 +36,11 @@ struct NhScal {
   unsigned long long lam_bits;  // max over cells of the CFL rate, as the bits of a non-negative double
   long long steps, iters_total, clamps, solves;
   int iters_last, iters_max, flags, pad;
+  // solver 1 (nh_solver.cu, k_srj): bits of non-negative doubles, reduced by integer atomicMax
+  unsigned long long srj_rho_bits;   // Gershgorin radius of D^-1 A about 1 (k_scale_rows)
+  unsigned long long srj_bmax_bits;  // max |b / A_C| (k_scale_rows)
+  unsigned long long srj_E_bits[3];  // max |Jacobi increment| of sweep k in slot k % 3
+  int srj_bad, pad2;                 // a NaN appeared in a sweep
 };
 
 enum { NH_FLAG_NOCONV = 1, NH_FLAG_NAN = 2, NH_FLAG_BADSTATE = 4 };
@@ -139,6 +144,8 @@ struct nh_ctx {
   std::vector<void*> raw;  // allocation bases (node planes are handed out offset to node (0,0))
   double* part;  // per-CTA partial sums of the solver
   int solver_grid, solver_occ, solver_nstrips, solver_R, solver_nbands;
+  int srj_grid, srj_R, srj_nbands;  // solver 1: cooperative grid and band height of k_srj
+  double* srj_cos;                  // solver 1: cos(pi (2 perm_i - 1) / 2M), tables of M = 1, 2, 4, ... at offset M - 1
   size_t nni;  // doubles per internal node plane (ghost ring included)
   NhScal* sc;       // device scalars
   NhScal* sc_host;  // pinned mirror
@@ -166,7 +173,8 @@ void nh_launch_breaking(nh_ctx* c, const double* h, const double* qx1, const dou
 void nh_launch_rhs(nh_ctx* c, const double* h, const double* qx, const double* qy, const double* z,
                    const double* w, double* b, int constraint_only);
 void nh_launch_coeffs(nh_ctx* c, const double* h, const double* z);  // -> dg, dinv, raw cE..cS
-void nh_launch_scale_coeffs(nh_ctx* c);  // cX *= dinv(neighbour); ghost lines <- (swapped) images
+void nh_launch_scale_coeffs(nh_ctx* c);  // solver 0: cX *= dinv(neighbour)
+void nh_launch_scale_rows(nh_ctx* c, const double* b, double* bp);  // solver 1: cX *= dinv, bp = b dinv, rho, max|bp|
 void nh_launch_apply_A(nh_ctx* c, const double* h, const double* z, const double* x, double* y);
 void nh_launch_correct(nh_ctx* c, const double* h, const double* z, const double* qx2,
                        const double* qy2, const double* w2, const double* p, double* qx_out,

@@ -120,6 +120,40 @@ k_scale_coeffs(NhGrid G, const double* __restrict__ dinv, double* __restrict__ c
   cS[k] = cS[k] * F.node(dinv, I, J - 1);
 }
 
+// Row scaling for solver 1 (the paper's Jacobi method, R28): c_X = A_X / A_C, b' = b / A_C; the
+// Gershgorin radius rho = max_n ((|c_E|+|c_W|)+|c_N|)+|c_S| and max |b'| are reduced exactly
+// (max of non-negative doubles = integer max of their bit patterns).
+__global__ void __launch_bounds__(BX* BY)
+k_scale_rows(NhGrid G, const double* __restrict__ dinv, double* __restrict__ cE,
+             double* __restrict__ cW, double* __restrict__ cN, double* __restrict__ cS,
+             const double* __restrict__ b, double* __restrict__ bp, NhScal* sc) {
+  int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
+  double rad = 0.0, bm = 0.0;
+  if (I < G.nnx && J < G.nny) {
+    size_t k = (size_t)J * G.np + I;
+    double di = dinv[k];
+    double e = cE[k] * di, w = cW[k] * di, n = cN[k] * di, s = cS[k] * di;
+    cE[k] = e; cW[k] = w; cN[k] = n; cS[k] = s;
+    double v = b[k] * di;
+    bp[k] = v;
+    rad = ((fabs(e) + fabs(w)) + fabs(n)) + fabs(s);
+    bm = fabs(v);
+  }
+  // NaN sorts above every finite pattern, so a NaN in b' or in a coefficient survives the max
+  unsigned long long rb = (unsigned long long)__double_as_longlong(rad);
+  unsigned long long bb = (unsigned long long)__double_as_longlong(bm);
+  for (int o = 16; o > 0; o >>= 1) {
+    unsigned long long t = __shfl_xor_sync(0xffffffffu, rb, o);
+    rb = t > rb ? t : rb;
+    t = __shfl_xor_sync(0xffffffffu, bb, o);
+    bb = t > bb ? t : bb;
+  }
+  if (((threadIdx.y * BX + threadIdx.x) & 31) == 0) {
+    if (rb) atomicMax(&sc->srj_rho_bits, rb);
+    if (bb) atomicMax(&sc->srj_bmax_bits, bb);
+  }
+}
+
 // y = A x on the distinct nodes, coefficients recomputed from (h, z) on the fly (matrix-free,
 // L535-537); neighbours through the node maps (R10).
 __global__ void __launch_bounds__(BX* BY)
@@ -378,6 +412,11 @@ void nh_launch_coeffs(nh_ctx* c, const double* h, const double* z) {
 void nh_launch_scale_coeffs(nh_ctx* c) {
   k_scale_coeffs<<<grid2(c->g.nnx, c->g.nny), dim3(BX, BY), 0, c->stream>>>(c->g, c->dinv, c->cE,
                                                                            c->cW, c->cN, c->cS);
+  c->launches++;
+}
+void nh_launch_scale_rows(nh_ctx* c, const double* b, double* bp) {
+  k_scale_rows<<<grid2(c->g.nnx, c->g.nny), dim3(BX, BY), 0, c->stream>>>(
+      c->g, c->dinv, c->cE, c->cW, c->cN, c->cS, b, bp, c->sc);
   c->launches++;
 }
 void nh_launch_apply_A(nh_ctx* c, const double* h, const double* z, const double* x, double* y) {

@@ -520,6 +520,140 @@ __global__ void __launch_bounds__(NT, 2) k_bicgstab(SolveP P) {
   }
 }
 
+// ---- solver 1: the paper's Jacobi method with scheduled relaxation (L507-514, L535-539; R28) ----
+// One persistent cooperative kernel per solve; one sweep and one grid barrier per iteration, no dot
+// products.  Sweep k:  z = b' - (x + ((c_E x_E + c_W x_W) + c_N x_N) + c_S x_S)  (the increment of
+// the plain Jacobi method), E_k = max |z| (eq. (32)), x' = x + omega_k z, with the row-scaled
+// coefficients and b' of k_scale_rows.  Every operation is a plain IEEE multiply / add in the
+// order the oracle uses (no FMA), a max is exact, and a Jacobi sweep does not depend on the sweep
+// order: the iterates, the iteration count and E are bit-identical to the CPU oracle's.
+// Traffic: reads x, b', 4 c; writes x': 7 doubles = 56 B per node-iteration.
+struct SrjP {
+  NhGrid G;
+  int nstrips, R, nbands;
+  const double *cE, *cW, *cN, *cS, *bp, *costab;
+  double *xA, *xB;  // xA = the pressure plane p (start and result), xB = scratch
+  NhScal* sc;
+  double eps;
+  int maxit, mmax, count_stats;
+};
+
+__device__ __forceinline__ void srj_sweep(const SrjP& P, const SolveP& Q, double om, const double* x,
+                                          double* xn, unsigned long long* Eslot) {
+  const NhGrid& G = P.G;
+  const int lane = threadIdx.x & 31;
+  const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
+  const int nunits = P.nstrips * P.nbands;
+  double emax = 0.0;
+  bool bad = false;
+  struct Row { double2 xn, b, e, w, n, s; };
+  for (int u = gw; u < nunits; u += tw) {
+    Unit U = make_unit(Q, u, lane);
+    double2 xm = ld2(x, G, U.c0, U.Ja - 1), xc = ld2(x, G, U.c0, U.Ja);
+    auto ld_row = [&](Row& X, int j) {  // operands of sweep step j (x of row j+1, the rest of row j)
+      X.xn = ld2(x, G, U.c0, min(j + 1, U.Jb));
+      const int jc = min(j, U.Jb - 1);
+      X.b = ld2(P.bp, G, U.c0, jc);
+      X.e = ld2(P.cE, G, U.c0, jc); X.w = ld2(P.cW, G, U.c0, jc);
+      X.n = ld2(P.cN, G, U.c0, jc); X.s = ld2(P.cS, G, U.c0, jc);
+    };
+    auto step = [&](int j, Row& cur, Row& nxt) {
+      ld_row(nxt, j + 1);  // request the next step's operands first
+      double west0 = __shfl_up_sync(0xffffffffu, xc.y, 1);
+      double east1 = __shfl_down_sync(0xffffffffu, xc.x, 1);
+      double ax0 = xc.x + (((cur.e.x * xc.y + cur.w.x * west0) + cur.n.x * cur.xn.x) + cur.s.x * xm.x);
+      double ax1 = xc.y + (((cur.e.y * east1 + cur.w.y * xc.x) + cur.n.y * cur.xn.y) + cur.s.y * xm.y);
+      double z0 = cur.b.x - ax0, z1 = cur.b.y - ax1;
+      if (U.own0) { emax = fmax(emax, fabs(z0)); bad |= !(z0 == z0); }
+      if (U.own1) { emax = fmax(emax, fabs(z1)); bad |= !(z1 == z1); }
+      st2(xn, Q, U, j, make_double2(xc.x + om * z0, xc.y + om * z1));
+      xm = xc; xc = cur.xn;
+    };
+    Row A, B;
+    ld_row(A, U.Ja);
+    for (int j = U.Ja; j < U.Jb; j += 2) {
+      step(j, A, B);
+      if (j + 1 < U.Jb) step(j + 1, B, A);
+    }
+  }
+  // CTA max -> one integer atomicMax (exact, order independent)
+  for (int o = 16; o > 0; o >>= 1) emax = fmax(emax, __shfl_xor_sync(0xffffffffu, emax, o));
+  __shared__ double wmax[NW];
+  if (lane == 0) wmax[threadIdx.x >> 5] = emax;
+  int anybad = __syncthreads_or(bad);
+  if (threadIdx.x == 0) {
+    double m = 0.0;
+#pragma unroll
+    for (int w = 0; w < NW; ++w) m = fmax(m, wmax[w]);
+    if (m > 0.0) atomicMax(Eslot, (unsigned long long)__double_as_longlong(m));
+    if (anybad) atomicOr(&P.sc->srj_bad, 1);
+  }
+}
+
+__global__ void __launch_bounds__(NT, 2) k_srj(SrjP P) {
+  cg::grid_group grid = cg::this_grid();
+  const NhGrid& G = P.G;
+  NhScal* sc = P.sc;
+  SolveP Q;  // geometry view for make_unit / st2
+  Q.G = P.G; Q.nstrips = P.nstrips; Q.R = P.R; Q.nbands = P.nbands;
+  const double rho = __longlong_as_double((long long)sc->srj_rho_bits);
+  const double bmax = __longlong_as_double((long long)sc->srj_bmax_bits);
+  int iters = 0, status = 0;
+  double E = 0.0;
+  double *x = P.xA, *xn = P.xB;
+  if (!(bmax == bmax) || isinf(bmax)) {
+    status = NH_ENAN;
+  } else if (bmax == 0.0) {  // b = 0 => p~ = 0, zero iterations (same convention as solver 0)
+    for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
+      for (int I = threadIdx.x; I < G.nnx; I += NT) P.xA[nidx(G, I, J)] = 0.0;
+  } else if (!(rho < 1.0)) {
+    status = NH_ENOCONV;  // not strictly diagonally dominant: no bound on the spectrum
+  } else {
+    // cycle length: smallest power of two with M sqrt(2 (1 - rho)) >= 7.6, at most mmax
+    const double gap = sqrt(2.0 * (1.0 - rho));
+    int M = 1;
+    while (M < P.mmax && (double)M * gap < 7.6) M *= 2;
+    const double* cosv = P.costab + (M - 1);
+    // ghost images of the start vector
+    for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
+      for (int I = threadIdx.x; I < G.nnx; I += NT) store_images(G, x, I, J, x[nidx(G, I, J)]);
+    grid.sync();
+    for (;;) {
+      const double om = 1.0 / (1.0 - rho * cosv[iters % M]);
+      unsigned long long* slot = &sc->srj_E_bits[iters % 3];
+      srj_sweep(P, Q, om, x, xn, slot);
+      grid.sync();
+      E = __longlong_as_double((long long)__ldcg(slot));
+      const int bad = __ldcg(&sc->srj_bad);
+      if (blockIdx.x == 0 && threadIdx.x == 0) sc->srj_E_bits[(iters + 2) % 3] = 0ULL;
+      if (bad) { status = NH_ENAN; break; }
+      if (E < P.eps) break;  // eq. (32): x is the accepted iterate
+      if (iters >= P.maxit) { status = NH_ENOCONV; break; }
+      double* t = x; x = xn; xn = t;
+      iters++;
+    }
+    if (x != P.xA) {  // the accepted iterate lives in the scratch plane
+      for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
+        for (int I = threadIdx.x; I < G.nnx; I += NT) P.xA[nidx(G, I, J)] = x[nidx(G, I, J)];
+    }
+  }
+  grid.sync();
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    if (status == NH_ENOCONV) sc->flags |= NH_FLAG_NOCONV;
+    if (status == NH_ENAN) sc->flags |= NH_FLAG_NAN;
+    sc->iters_last = iters;
+    sc->res_last = E;
+    if (P.count_stats) {
+      sc->iters_total += iters;
+      sc->solves += 1;
+      if (iters > sc->iters_max) sc->iters_max = iters;
+    }
+    // reset the reductions for the next solve
+    sc->srj_rho_bits = 0ULL; sc->srj_bmax_bits = 0ULL; sc->srj_bad = 0;
+    sc->srj_E_bits[0] = sc->srj_E_bits[1] = sc->srj_E_bits[2] = 0ULL;
+  }
+}
+
 }  // namespace
 
 // Cooperative grid (one wave of co-resident CTAs) and the band height R: every warp takes the
@@ -555,10 +689,66 @@ int nh_solver_setup(nh_ctx* c) {
   c->solver_nbands = (nny + bestR - 1) / bestR;
   e = cudaMalloc(&c->part, sizeof(double) * 2 * MAXDOT * (size_t)grid);
   if (e != cudaSuccess) return NH_ENOMEM;
+  c->srj_cos = nullptr;
+  if (c->prm.solver == 1) {
+    // solver 1: its own cooperative grid / band height, and the relaxation schedule:
+    // cos(pi (2 perm_i - 1) / 2M) in Lebedev-Finogenov order for M = 1, 2, 4, ..., mmax (R28),
+    // evaluated on the host so that the factors are the ones a CPU evaluation produces.
+    int occ1 = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_srj, NT, 0);
+    if (e != cudaSuccess || occ1 < 1) {
+      snprintf(c->err, sizeof(c->err), "srj occupancy query failed: %s", cudaGetErrorString(e));
+      return NH_ECUDA;
+    }
+    long long g1 = (long long)occ1 * c->sm_count;
+    if (g1 > (small_units + NW - 1) / NW) g1 = (small_units + NW - 1) / NW;
+    if (g1 < 1) g1 = 1;
+    const long long tw1 = g1 * NW;
+    int R1 = nny;
+    long long best1 = -1;
+    for (int R = 4; R <= nny; ++R) {
+      long long nb = (nny + R - 1) / R;
+      long long rounds = (nstrips * nb + tw1 - 1) / tw1;
+      long long cost = rounds * (R + 2);
+      if (best1 < 0 || cost < best1) { best1 = cost; R1 = R; }
+    }
+    if (nny < 4) R1 = nny;
+    c->srj_grid = (int)g1; c->srj_R = R1; c->srj_nbands = (nny + R1 - 1) / R1;
+    const int mmax = c->prm.srj_mmax;
+    std::vector<double> tab((size_t)2 * mmax - 1);
+    std::vector<int> perm((size_t)mmax);
+    for (int M = 1; M <= mmax; M *= 2) {
+      perm[0] = 1;
+      for (int m = 1; m < M; m *= 2)
+        for (int i = m - 1; i >= 0; --i) {
+          int a = perm[i];
+          perm[2 * i] = a; perm[2 * i + 1] = 2 * m + 1 - a;
+        }
+      for (int i = 0; i < M; ++i)
+        tab[(size_t)(M - 1) + i] = cos(3.14159265358979323846 * (double)(2 * perm[i] - 1) / (double)(2 * M));
+    }
+    e = cudaMalloc(&c->srj_cos, sizeof(double) * tab.size());
+    if (e != cudaSuccess) return NH_ENOMEM;
+    e = cudaMemcpy(c->srj_cos, tab.data(), sizeof(double) * tab.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return NH_ECUDA;
+  }
   return NH_OK;
 }
 
 void nh_launch_solve(nh_ctx* c, const double* b, double* x, int count_stats) {
+  if (c->prm.solver == 1) {  // b is c->kr = b / A_C here (nh_launch_scale_rows)
+    SrjP S;
+    S.G = c->g;
+    S.nstrips = c->solver_nstrips; S.R = c->srj_R; S.nbands = c->srj_nbands;
+    S.cE = c->cE; S.cW = c->cW; S.cN = c->cN; S.cS = c->cS; S.bp = c->kr; S.costab = c->srj_cos;
+    S.xA = x; S.xB = c->ky; S.sc = c->sc; S.eps = c->prm.srj_eps;
+    S.maxit = c->prm.solver_maxit; S.mmax = c->prm.srj_mmax; S.count_stats = count_stats;
+    void* args[] = {&S};
+    NH_CUDA_OK(c, cudaLaunchCooperativeKernel((void*)k_srj, dim3(c->srj_grid), dim3(NT), args, 0,
+                                              c->stream));
+    c->launches++;
+    return;
+  }
   SolveP P;
   P.G = c->g;
   P.nstrips = c->solver_nstrips; P.R = c->solver_R; P.nbands = c->solver_nbands;

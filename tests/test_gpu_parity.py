@@ -392,3 +392,68 @@ def test_manning_negative_coefficient_is_rejected(G):
     with pytest.raises(G.NHError) as e:
         G.NH(8, 8, 1.0, 1.0, np.ones((8, 8)), manning_n=-1.0)
     assert e.value.code == G.EINVAL
+
+
+# ---------------------------------------------------------------- solver 1: the paper's Jacobi
+# method with scheduled relaxation (R28).  No dot products, a max-norm stopping rule and plain
+# multiply / add arithmetic in the oracle's order: everything is compared BIT-EXACTLY, iteration
+# counts included.
+@pytest.mark.parametrize("bcs", BCS)
+@pytest.mark.parametrize("dry", [0.0, 0.3])
+def test_srj_solve_bit_exact(O, G, bcs, dry):
+    cfg = rnd_cfg(150, 77, bcs, seed=41, dry=dry, dx=0.2, dy=0.25, solver=1, srj_eps=1e-10)
+    o, g = both(O, G, cfg)
+    b = o.rhs(0.01)
+    xo, ito, Eo = o.solve(b, x0=cfg["p"])
+    xg, itg, Eg = g.solve(b, x0=cfg["p"])
+    assert ito == itg and ito >= 5 and Eo == Eg and Eg < 1e-10
+    assert np.array_equal(xo, xg)
+
+
+@pytest.mark.parametrize("bcs", [BCS[0], BCS[2]])
+@pytest.mark.parametrize("eps", [1e-5, 1e-12])
+def test_srj_full_steps_bit_exact(O, G, bcs, eps):
+    cfg = rnd_cfg(90, 64, bcs, seed=43, dry=0.2, dx=0.1, dy=0.1, solver=1, srj_eps=eps,
+                  breaking=1, B1=0.02, B2=0.05)
+    o, g = both(O, G, cfg)
+    o.step(3)
+    g.step(3)
+    assert g.sync() == 0
+    so, sg = o.get_state(), g.get_state()
+    for k in so:
+        assert np.array_equal(so[k], sg[k]), k
+    io, ig = o.info(), g.info()
+    assert io.iters_total == ig.iters_total > 0 and io.res_last == ig.res_last and io.t == ig.t
+
+
+def test_srj_config5_crop_and_config3_bit_exact_and_close_to_bicgstab(O, G):
+    for idx, kw in ((5, dict(nx=192, ny=160)), (3, dict(nx=160, ny=128))):
+        cfg = inputs.make_config(idx, **kw)
+        o, g = both(O, G, cfg, solver=1, srj_eps=1e-12)
+        o.step(2)
+        g.step(2)
+        assert g.sync() == 0
+        so, sg = o.get_state(), g.get_state()
+        for k in so:
+            assert np.array_equal(so[k], sg[k]), (idx, k)
+        assert o.info().iters_total == g.info().iters_total
+        _, gb = both(O, G, cfg)          # solver 0 on the GPU: same physics within the tolerances
+        gb.step(2)
+        assert gb.sync() == 0
+        assert_parity(sg, gb.get_state(), cfg["H"], cfg["h0"], tol=1e-8)
+
+
+def test_srj_zero_rhs_nonconvergence_and_bad_parameters(O, G):
+    cfg = inputs.make_config(2, nx=96, ny=80)
+    _, g = both(O, G, cfg, solver=1)
+    g.step(2)
+    assert g.sync() == 0 and g.info().iters_total == 0 and np.all(g.get_state()["p"] == 0.0)
+    cfg = rnd_cfg(64, 48, BCS[1], seed=47, solver=1, srj_eps=1e-13, solver_maxit=5)
+    o, g = both(O, G, cfg)
+    b = o.rhs(0.01)
+    xg, itg, Eg = g.solve(b, allow=(G.ENOCONV,))
+    xo, ito, Eo = o.solve(b, allow_noconv=True)
+    assert itg == ito == 5 and np.array_equal(xg, xo)
+    for bad in (dict(solver=3), dict(solver=1, srj_mmax=100), dict(solver=1, srj_eps=-1.0)):
+        with pytest.raises(G.NHError):
+            G.NH(8, 8, 1.0, 1.0, np.ones((8, 8)), **bad)
