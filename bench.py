@@ -193,7 +193,10 @@ def run_b200(args):
     nx, ny = cfg["nx"], cfg["ny"]
     nc, nn = nx * ny, (nx + 1) * (ny + 1)
     stream = torch.cuda.Stream(device=dev)
-    sim = nh.NH(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], stream=stream, **cfg["params"])
+    prm = dict(cfg["params"])
+    if args.solver == "srj":
+        prm.update(solver=1, srj_eps=args.srj_eps)
+    sim = nh.NH(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], stream=stream, **prm)
     sim.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
 
     # ---- device-resident leg: W warm-up steps, then exactly K timed steps
@@ -227,21 +230,27 @@ def run_b200(args):
     peak, peak_src = _peaks()
     sol_ms, sol_n = prof["solver"]
     node_iters = (iters + solves) * float(nn)          # + the polish iteration of every solve
-    achieved = BYTES_PER_NODE_ITER * node_iters / (sol_ms * 1e-3) / 1e9 if sol_ms > 0 else 0.0
+    bytes_unit = BYTES_PER_NODE_ITER
+    if args.solver == "srj":   # one Jacobi sweep: reads x, b', 4 coefficients, writes x'
+        bytes_unit = 56.0
+        node_iters = (iters + solves) * float(nn)      # + the sweep that meets the stopping rule
+    achieved = bytes_unit * node_iters / (sol_ms * 1e-3) / 1e9 if sol_ms > 0 else 0.0
     traffic = None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
         try:
             tj = json.load(open(tp))
-            if tj.get("workload") == cfg["name"] and tj.get("nx") == nx and tj.get("ny") == ny:
+            if tj.get("workload") == cfg["name"] and tj.get("nx") == nx and tj.get("ny") == ny \
+                    and args.solver == "bicgstab":
                 traffic = tj.get("dram_bytes_per_launch")
         except Exception:
             pass
     roofline = {
-        "bound": "hbm", "kernel": "k_bicgstab (one cooperative launch per pressure solve)",
+        "bound": "hbm", "kernel": ("k_srj" if args.solver == "srj" else "k_bicgstab") +
+                                  " (one cooperative launch per pressure solve)",
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
         "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0,
-        "bytes_per_node_iteration": BYTES_PER_NODE_ITER, "launches": sol_n,
+        "bytes_per_node_iteration": bytes_unit, "launches": sol_n,
         "avg_launch_ms": sol_ms / max(sol_n, 1),
         "iterations_per_launch": (iters + solves) / max(solves, 1),
         "phase_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
@@ -278,7 +287,8 @@ def run_b200(args):
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": f"configs[{args.config - 1}] {cfg['name']} {nx}x{ny} cells, dx={cfg['dx']} m",
-                   "solver": "Jacobi-BiCGStab rtol 1e-12, device-resident convergence",
+                   "solver": ("Jacobi-BiCGStab rtol 1e-12, device-resident convergence" if args.solver == "bicgstab"
+                              else f"scheduled-relaxation Jacobi (paper's solver), increment rule (32) eps {args.srj_eps:g}"),
                    "iters_per_solve": iters / max(solves, 1), "time_order": 2,
                    "l2": "working set >> L2 (one fp64 plane = %.0f MB); no flush needed" % (8e-6 * nc)
                          if 8 * nc > 200e6 else "working set near/below L2 size: L2-resident, not an HBM claim",
@@ -311,6 +321,9 @@ def main():
     ap.add_argument("--nx", type=int, default=0)
     ap.add_argument("--ny", type=int, default=0)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--solver", default="bicgstab", choices=["bicgstab", "srj"],
+                    help="bicgstab: north_star solver (default); srj: the paper's scheduled-relaxation Jacobi")
+    ap.add_argument("--srj-eps", type=float, default=1e-5, help="stopping tolerance of eq. (32) for --solver srj")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -550,7 +550,8 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
  *   - M = smallest power of two with M sqrt(2 (1-rho)) >= 7.6 (one cycle then damps every mode
  *     about 1000-fold), at most srj_mmax;
  *   - iteration k: z = b' - (x + c_E x_E + c_W x_W + c_N x_N + c_S x_S) is the increment of the
- *     plain Jacobi method; stop if E = ||z||_inf < srj_eps, eq. (32) (x is then the answer);
+ *     plain Jacobi method; stop if E = ||z||_inf < tol, eq. (32) (x is then the answer), with
+ *     tol = srj_eps (the paper's absolute epsilon) or, if srj_rel > 0, tol = srj_rel max|b'|;
  *     otherwise x <- x + omega z.  No dot products; every node update depends on x of the
  *     previous sweep only, so the result does not depend on the sweep order.
  * x: start -> solution.  res_out = the last E. */
@@ -607,6 +608,8 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
   }
   int iters = 0, status = NHO_OK;
   double E = 0.0;
+  /* tolerance of (32): absolute (the paper's epsilon), or relative to max |b'| (R28) */
+  const double tol = (c->prm.srj_rel > 0.0) ? c->prm.srj_rel * bmax : c->prm.srj_eps;
   for (;;) {
     const double om = omega[iters % M];
     double Emax = 0.0;
@@ -625,7 +628,7 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
       }
     E = Emax;
     if (nan) { status = NHO_ENAN; break; }
-    if (E < c->prm.srj_eps) break;               /* eq. (32): x is the accepted iterate */
+    if (E < tol) break;                          /* eq. (32): x is the accepted iterate */
     if (iters >= maxit) { status = NHO_ENOCONV; break; }
 #pragma omp parallel for if (c->ny >= 48) schedule(static)
     for (int J = 0; J < nny; ++J)
@@ -860,6 +863,7 @@ int nho_create(nho_ctx** out, int nx, int ny, double dx, double dy, const double
   if (prm->precision != 64) return NHO_EINVAL;
   if (!(prm->manning_n >= 0.0)) return NHO_EINVAL;
   if (prm->solver != 0 && prm->solver != 1) return NHO_EINVAL;
+  if (!(prm->srj_rel >= 0.0)) return NHO_EINVAL;
   if (prm->solver == 1 && (!(prm->srj_eps > 0.0) || prm->srj_mmax < 1 || prm->srj_mmax > 4096 ||
                            (prm->srj_mmax & (prm->srj_mmax - 1)) != 0)) return NHO_EINVAL;
   if (prm->breaking && !(prm->B1 > 0.0 && prm->B2 > 0.0)) return NHO_EINVAL;

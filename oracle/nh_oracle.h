@@ -36,6 +36,7 @@ typedef struct {
   double gen_A, gen_h0, gen_x0, gen_Lrel; /* solitary-wave generating zone at x-lo (L417-431, R18) */
   double manning_n;    /* Gauckler-Manning coefficient n (L61-65, L773-775); 0 = frictionless     */
   double srj_eps;      /* solver 1: stop when the Jacobi increment of (32) is < srj_eps (L507-514) */
+  double srj_rel;      /* solver 1: if > 0 the tolerance of (32) is srj_rel * max|b/A_C| instead    */
   int breaking;        /* 1: eddy-viscosity breaking sources on (section 3)             */
   int nonhydro;        /* 0: hydrostatic SWE path only (p = 0, w frozen)                */
   int time_order;      /* 1 or 2 (TVD RK2, L406, L516)                                  */

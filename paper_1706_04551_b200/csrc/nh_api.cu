@@ -230,6 +230,7 @@ int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* 
   if (prm->precision != 64) return NH_EINVAL;
   if (!(prm->manning_n >= 0.0)) return NH_EINVAL;
   if (prm->solver != 0 && prm->solver != 1) return NH_EINVAL;
+  if (!(prm->srj_rel >= 0.0)) return NH_EINVAL;
   if (prm->solver == 1 && (!(prm->srj_eps > 0.0) || prm->srj_mmax < 1 || prm->srj_mmax > 4096 ||
                            (prm->srj_mmax & (prm->srj_mmax - 1)) != 0)) return NH_EINVAL;
   if (prm->breaking && !(prm->B1 > 0.0 && prm->B2 > 0.0)) return NH_EINVAL;

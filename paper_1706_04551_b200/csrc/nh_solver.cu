@@ -534,7 +534,7 @@ struct SrjP {
   const double *cE, *cW, *cN, *cS, *bp, *costab;
   double *xA, *xB;  // xA = the pressure plane p (start and result), xB = scratch
   NhScal* sc;
-  double eps;
+  double eps, rel;  // tolerance of (32): eps, or rel * max|b'| when rel > 0
   int maxit, mmax, count_stats;
 };
 
@@ -614,6 +614,7 @@ __global__ void __launch_bounds__(NT, 2) k_srj(SrjP P) {
     int M = 1;
     while (M < P.mmax && (double)M * gap < 7.6) M *= 2;
     const double* cosv = P.costab + (M - 1);
+    const double tol = (P.rel > 0.0) ? P.rel * bmax : P.eps;
     // ghost images of the start vector
     for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
       for (int I = threadIdx.x; I < G.nnx; I += NT) store_images(G, x, I, J, x[nidx(G, I, J)]);
@@ -627,7 +628,7 @@ __global__ void __launch_bounds__(NT, 2) k_srj(SrjP P) {
       const int bad = __ldcg(&sc->srj_bad);
       if (blockIdx.x == 0 && threadIdx.x == 0) sc->srj_E_bits[(iters + 2) % 3] = 0ULL;
       if (bad) { status = NH_ENAN; break; }
-      if (E < P.eps) break;  // eq. (32): x is the accepted iterate
+      if (E < tol) break;  // eq. (32): x is the accepted iterate
       if (iters >= P.maxit) { status = NH_ENOCONV; break; }
       double* t = x; x = xn; xn = t;
       iters++;
@@ -741,7 +742,7 @@ void nh_launch_solve(nh_ctx* c, const double* b, double* x, int count_stats) {
     S.G = c->g;
     S.nstrips = c->solver_nstrips; S.R = c->srj_R; S.nbands = c->srj_nbands;
     S.cE = c->cE; S.cW = c->cW; S.cN = c->cN; S.cS = c->cS; S.bp = c->kr; S.costab = c->srj_cos;
-    S.xA = x; S.xB = c->ky; S.sc = c->sc; S.eps = c->prm.srj_eps;
+    S.xA = x; S.xB = c->ky; S.sc = c->sc; S.eps = c->prm.srj_eps; S.rel = c->prm.srj_rel;
     S.maxit = c->prm.solver_maxit; S.mmax = c->prm.srj_mmax; S.count_stats = count_stats;
     void* args[] = {&S};
     NH_CUDA_OK(c, cudaLaunchCooperativeKernel((void*)k_srj, dim3(c->srj_grid), dim3(NT), args, 0,

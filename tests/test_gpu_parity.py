@@ -457,3 +457,19 @@ def test_srj_zero_rhs_nonconvergence_and_bad_parameters(O, G):
     for bad in (dict(solver=3), dict(solver=1, srj_mmax=100), dict(solver=1, srj_eps=-1.0)):
         with pytest.raises(G.NHError):
             G.NH(8, 8, 1.0, 1.0, np.ones((8, 8)), **bad)
+
+
+def test_srj_relative_tolerance_bit_exact(O, G):
+    cfg = rnd_cfg(120, 50, BCS[3], seed=53, dry=0.1, dx=0.1, dy=0.1, solver=1, srj_rel=1e-9)
+    o, g = both(O, G, cfg)
+    o.step(2)
+    g.step(2)
+    assert g.sync() == 0
+    so, sg = o.get_state(), g.get_state()
+    for k in so:
+        assert np.array_equal(so[k], sg[k]), k
+    assert o.info().iters_total == g.info().iters_total > 0
+    # and the rule is what it says: E < srj_rel max|b / A_C| at exit, so a tighter srj_rel iterates longer
+    _, g2 = both(O, G, cfg, srj_rel=1e-12)
+    g2.step(2)
+    assert g2.sync() == 0 and g2.info().iters_total > g.info().iters_total

@@ -747,3 +747,20 @@ def test_srj_zero_rhs_gives_zero_pressure_and_bad_parameters_are_rejected(O):
     for bad in (dict(solver=2), dict(solver=1, srj_mmax=48), dict(solver=1, srj_eps=0.0)):
         with pytest.raises(O.OracleError):
             O.Oracle(8, 8, 1.0, 1.0, np.ones((8, 8)), **bad)
+
+
+def test_srj_relative_rule_bounds_the_scaled_residual(O):
+    # srj_rel: stop at max|D^-1 (b - A x)| < srj_rel max|D^-1 b|; checked with the dense matrix
+    nx, ny, dx, dy = 10, 8, 0.3, 0.3
+    st = inputs.random_smooth_state(nx, ny, dx, dy, seed=4, depth=1.0, rough=0.3)
+    o = O.Oracle(nx, ny, dx, dy, st["H"], bc_xlo=WALL, bc_xhi=WALL, bc_ylo=OUT, bc_yhi=OUT,
+                 solver=1, srj_rel=1e-8)
+    o.set_state(st["h"], st["qx"], st["qy"], st["w"])
+    A, nnx, nny = dense_A(o, ny, nx, False, False)
+    b = o.rhs(0.01)
+    x, it, E = o.solve(b)
+    D = np.diag(A)
+    z = (b.ravel() - A @ x.ravel()) / D
+    bmax = np.max(np.abs(b.ravel() / D))
+    assert it > 3 and np.max(np.abs(z)) < 1e-8 * bmax * (1 + 1e-6)
+    assert abs(E - np.max(np.abs(z))) <= 1e-3 * E
