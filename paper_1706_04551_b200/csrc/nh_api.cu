@@ -159,10 +159,13 @@ void nonhydro_part(nh_ctx* c, const double* h1, const double* qx1, const double*
       qxs = c->qx2; qys = c->qy2; ws = c->w2;
     }
     nh_launch_compute_z(c, h1, c->z);
-    nh_launch_rhs(c, h1, qxs, qys, c->z, ws, c->b, 0);
-    nh_launch_coeffs(c, h1, c->z);
-    if (c->prm.solver == 1) nh_launch_scale_rows(c, c->b, c->kr);
-    else nh_launch_scale_coeffs(c);
+    if (c->prm.solver == 1) {
+      nh_launch_assemble_rows(c, h1, qxs, qys, c->z, ws, c->kr);
+    } else {
+      nh_launch_rhs(c, h1, qxs, qys, c->z, ws, c->b, 0);
+      nh_launch_coeffs(c, h1, c->z);
+      nh_launch_scale_coeffs(c);
+    }
   }
   {
     ProfScope ps(c, NH_PROF_SOLVER);

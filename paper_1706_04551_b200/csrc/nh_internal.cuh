@@ -174,7 +174,9 @@ void nh_launch_rhs(nh_ctx* c, const double* h, const double* qx, const double* q
                    const double* w, double* b, int constraint_only);
 void nh_launch_coeffs(nh_ctx* c, const double* h, const double* z);  // -> dg, dinv, raw cE..cS
 void nh_launch_scale_coeffs(nh_ctx* c);  // solver 0: cX *= dinv(neighbour)
-void nh_launch_scale_rows(nh_ctx* c, const double* b, double* bp);  // solver 1: cX *= dinv, bp = b dinv, rho, max|bp|
+void nh_launch_scale_rows(nh_ctx* c, const double* b, double* bp);
+void nh_launch_assemble_rows(nh_ctx* c, const double* h, const double* qx, const double* qy,
+                             const double* z, const double* w, double* bp);  // solver 1: rhs + rows + scaling fused  // solver 1: cX *= dinv, bp = b dinv, rho, max|bp|
 void nh_launch_apply_A(nh_ctx* c, const double* h, const double* z, const double* x, double* y);
 void nh_launch_correct(nh_ctx* c, const double* h, const double* z, const double* qx2,
                        const double* qy2, const double* w2, const double* p, double* qx_out,

@@ -170,13 +170,11 @@ k_apply_A(NhGrid G, const double* __restrict__ h, const double* __restrict__ z,
 }
 
 // S7: discrete constraint B of (37)-(40) at node (I,J); b = -B/dt (R15).
-__global__ void __launch_bounds__(BX* BY)
-k_rhs(NhGrid G, const NhScal* sc, int constraint_only, const double* __restrict__ h,
-      const double* __restrict__ qx, const double* __restrict__ qy, const double* __restrict__ z,
-      const double* __restrict__ w, double* __restrict__ b) {
-  int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
-  if (I >= G.nnx || J >= G.nny) return;
-  Fld F{G};
+__device__ __forceinline__ double node_B(const Fld& F, const double* __restrict__ h,
+                                         const double* __restrict__ qx,
+                                         const double* __restrict__ qy,
+                                         const double* __restrict__ z, double wn, int I, int J) {
+  const NhGrid& G = F.G;
   double hn = F.hnode(h, I, J);
   double q1E = 0.5 * (F.xn(qx, I, J) + F.xn(qx, I, J - 1));
   double q1W = 0.5 * (F.xn(qx, I - 1, J) + F.xn(qx, I - 1, J - 1));
@@ -187,11 +185,61 @@ k_rhs(NhGrid G, const NhScal* sc, int constraint_only, const double* __restrict_
   double zN = 0.5 * (F.even(z, I, J) + F.even(z, I - 1, J));
   double zS = 0.5 * (F.even(z, I, J - 1) + F.even(z, I - 1, J - 1));
   double divq = (q1E - q1W) / G.dx + (q2N - q2S) / G.dy;
+  return hn * divq - 0.5 * (q1E + q1W) * (zE - zW) / G.dx - 0.5 * (q2N + q2S) * (zN - zS) / G.dy +
+         2.0 * hn * wn;
+}
+
+__global__ void __launch_bounds__(BX* BY)
+k_rhs(NhGrid G, const NhScal* sc, int constraint_only, const double* __restrict__ h,
+      const double* __restrict__ qx, const double* __restrict__ qy, const double* __restrict__ z,
+      const double* __restrict__ w, double* __restrict__ b) {
+  int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
+  if (I >= G.nnx || J >= G.nny) return;
+  Fld F{G};
   size_t k = (size_t)J * G.np + I;
-  double B = hn * divq - 0.5 * (q1E + q1W) * (zE - zW) / G.dx -
-             0.5 * (q2N + q2S) * (zN - zS) / G.dy + 2.0 * hn * w[k];
+  double B = node_B(F, h, qx, qy, z, w[k], I, J);
   const double dt = sc->dt;
   b[k] = constraint_only ? B : ((dt > 0.0) ? -B / dt : 0.0);  // R26: dt = 0 (all dry) => b = 0
+}
+
+// Solver 1, whole assembly of a stage in one kernel (k_rhs + k_coeffs + k_scale_rows with the same
+// arithmetic, 3 kernels and 11 plane round trips less): right-hand side, rows, row scaling,
+// Gershgorin radius and max |b'|.
+__global__ void __launch_bounds__(BX* BY)
+k_assemble_rows(NhGrid G, NhScal* sc, const double* __restrict__ h, const double* __restrict__ qx,
+                const double* __restrict__ qy, const double* __restrict__ z,
+                const double* __restrict__ w, double* __restrict__ cE, double* __restrict__ cW,
+                double* __restrict__ cN, double* __restrict__ cS, double* __restrict__ bp) {
+  int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
+  double rad = 0.0, bm = 0.0;
+  if (I < G.nnx && J < G.nny) {
+    Fld F{G};
+    size_t k = (size_t)J * G.np + I;
+    double AC, AE, AW, AN, AS;
+    node_coeffs(F, h, z, I, J, AC, AE, AW, AN, AS);
+    double B = node_B(F, h, qx, qy, z, w[k], I, J);
+    const double dt = sc->dt;
+    double bv = (dt > 0.0) ? -B / dt : 0.0;
+    double di = 1.0 / AC;
+    double e = AE * di, ww = AW * di, n = AN * di, s = AS * di;
+    cE[k] = e; cW[k] = ww; cN[k] = n; cS[k] = s;
+    double v = bv * di;
+    bp[k] = v;
+    rad = ((fabs(e) + fabs(ww)) + fabs(n)) + fabs(s);
+    bm = fabs(v);
+  }
+  unsigned long long rb = (unsigned long long)__double_as_longlong(rad);
+  unsigned long long bb = (unsigned long long)__double_as_longlong(bm);
+  for (int o = 16; o > 0; o >>= 1) {
+    unsigned long long t = __shfl_xor_sync(0xffffffffu, rb, o);
+    rb = t > rb ? t : rb;
+    t = __shfl_xor_sync(0xffffffffu, bb, o);
+    bb = t > bb ? t : bb;
+  }
+  if (((threadIdx.y * BX + threadIdx.x) & 31) == 0) {
+    if (rb) atomicMax(&sc->srj_rho_bits, rb);
+    if (bb) atomicMax(&sc->srj_bmax_bits, bb);
+  }
 }
 
 // S6: breaking sources at cells (section 3, eqs (9)-(12); 2D reading R12): q** = q* + dt R_u
@@ -417,6 +465,12 @@ void nh_launch_scale_coeffs(nh_ctx* c) {
 void nh_launch_scale_rows(nh_ctx* c, const double* b, double* bp) {
   k_scale_rows<<<grid2(c->g.nnx, c->g.nny), dim3(BX, BY), 0, c->stream>>>(
       c->g, c->dinv, c->cE, c->cW, c->cN, c->cS, b, bp, c->sc);
+  c->launches++;
+}
+void nh_launch_assemble_rows(nh_ctx* c, const double* h, const double* qx, const double* qy,
+                             const double* z, const double* w, double* bp) {
+  k_assemble_rows<<<grid2(c->g.nnx, c->g.nny), dim3(BX, BY), 0, c->stream>>>(
+      c->g, c->sc, h, qx, qy, z, w, c->cE, c->cW, c->cN, c->cS, bp);
   c->launches++;
 }
 void nh_launch_apply_A(nh_ctx* c, const double* h, const double* z, const double* x, double* y) {
