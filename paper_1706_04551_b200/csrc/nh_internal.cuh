@@ -86,7 +86,10 @@ __device__ __forceinline__ double nh_dsg(double h, double q, double delta) {
   double h2 = h * h, h4 = h2 * h2;
   double d2 = delta * delta, d4 = d2 * d2;
   double den = sqrt(h4 + fmax(h4, d4));
-  return (NH_SQRT2 * h * q) / den;
+  double num = NH_SQRT2 * h * q;
+  // 0 / den = 0 (den > 0): same bits, but a zero dividend would send the fp64 division down its slow
+  // path, and still water is common (2.8 M of 3.5 M warp-divisions on the config-5 basin)
+  return (num == 0.0) ? num : num / den;
 }
 // R16: dinv(h) = sqrt(2) h / sqrt(h^4 + max(h^4, delta^4))  (= 1/h for h >= delta)
 __device__ __forceinline__ double nh_dinv_h(double h, double delta) {

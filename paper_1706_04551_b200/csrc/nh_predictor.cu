@@ -3,7 +3,8 @@
 //
 // One fused kernel does a1-a3: a (TX+4) x (TY+4) halo tile of the primitive fields (h, eta, u, v,
 // z_b) is staged in shared memory through the boundary index maps, then every thread owns one
-// cell, reconstructs, solves its four faces and writes U*.  No edge colouring, no accumulator
+// cell, reconstructs, solves the two faces on its high sides (handing D^+ to its neighbours
+// through shared memory) and writes U*.  No edge colouring, no accumulator
 // array (the paper's K1/K2 split, was made for write conflicts that a
 // cell-centric gather does not have).  Traffic: 4 planes read, 3 written = 56 B per cell.
 #include <math.h>
@@ -63,7 +64,9 @@ __device__ __forceinline__ void face_fluct(double g, double hm, double etam, dou
   double hh = 0.5 * (hm + hp);  // h_{i+1/2}, L276
   double sm = sqrt(hm), sp = sqrt(hp);
   double den = sm + sp;
-  double uh = (den > 0.0) ? (um * sm + up * sp) / den : 0.0;  // Roe average, L276; R4
+  double unum = um * sm + up * sp;
+  double uh = (den > 0.0) ? ((unum == 0.0) ? unum : unum / den) : 0.0;  // Roe average, L276; R4
+                                                    // (zero dividend: same bits, no slow path)
   double ch = sqrt(g * hh), cm = sqrt(g * hm), cp = sqrt(g * hp);
   double SL = fmin(uh - ch, um - cm);  // L290
   double SR = fmax(uh + ch, up + cp);  // L292
@@ -96,14 +99,38 @@ __device__ __forceinline__ void face_fluct(double g, double hm, double etam, dou
   }
 }
 
+// One face solve: the face between tile cell (lx,ly) and its neighbour in direction dir.
+// sL = slopes of the left / lower cell (returned: its owner needs them for the in-cell term).
+__device__ __forceinline__ void hi_face(const PredTile& T, int lx, int ly, int dir, int order,
+                                        double eps_dry, double g, double sL[4], double Dm[3],
+                                        double Dp[3]) {
+  const int di = (dir == 0), dj = (dir == 1);
+  Prim Pc = get_prim(T, lx, ly, dir);
+  Prim Pp = get_prim(T, lx + di, ly + dj, dir);
+  double sR[4];
+  cell_slopes(T, lx, ly, dir, order, eps_dry, sL);
+  cell_slopes(T, lx + di, ly + dj, dir, order, eps_dry, sR);
+  // S3 face states: left = c + s/2, right = p - s/2
+  double hL = Pc.h + 0.5 * sL[1], eL = Pc.eta + 0.5 * sL[0];
+  double uL = Pc.un + 0.5 * sL[2], vL = Pc.ut + 0.5 * sL[3];
+  double hR = Pp.h - 0.5 * sR[1], eR = Pp.eta - 0.5 * sR[0];
+  double uR = Pp.un - 0.5 * sR[2], vR = Pp.ut - 0.5 * sR[3];
+  face_fluct(g, hL, eL, uL, vL, hR, eR, uR, vR, Dm, Dp);
+}
+
+// Every face is solved once, by the thread of the cell on its low side, which keeps D^- for its
+// own update and publishes D^+ for its neighbour through shared memory; the faces on the low
+// edges of the tile (32 in y, 8 in x) are solved by the first 40 threads.  (The first version had
+// every cell solve its four faces and limit five cells: 2400 instructions per cell.)
 __global__ void __launch_bounds__(PTX* PTY)
 k_predictor(NhGrid G, double g, double delta, double eps_dry, double manning_n, int order,
-            const NhScal* sc,
-            const double* __restrict__ H, const double* __restrict__ h,
+            const NhScal* sc, const double* __restrict__ H, const double* __restrict__ h,
             const double* __restrict__ qx, const double* __restrict__ qy,
             double* __restrict__ h1, double* __restrict__ qx1, double* __restrict__ qy1,
             unsigned long long* clamps) {
   __shared__ PredTile T;
+  __shared__ double DPx[3][PTY][PTX + 1];  // D^+ of the x-face on the low side of cell lx - PH
+  __shared__ double DPy[3][PTY + 1][PTX];  // D^+ of the y-face on the low side of cell ly - PH
   const int i0 = blockIdx.x * PTX, j0 = blockIdx.y * PTY;
   const int tid = threadIdx.y * PTX + threadIdx.x;
   // S0 + S1: derived fields of the halo tile through the index maps
@@ -127,41 +154,57 @@ k_predictor(NhGrid G, double g, double delta, double eps_dry, double manning_n, 
   }
   __syncthreads();
   const int i = i0 + threadIdx.x, j = j0 + threadIdx.y;
-  if (i >= G.nx || j >= G.ny) return;
+  const bool active = (i < G.nx && j < G.ny);
   const int lx = threadIdx.x + PH, ly = threadIdx.y + PH;
+  double sown[2][4], Dm_hi[2][3];
+  if (active) {
+#pragma unroll
+    for (int dir = 0; dir < 2; ++dir) {
+      double Dp[3];
+      hi_face(T, lx, ly, dir, order, eps_dry, g, sown[dir], Dm_hi[dir], Dp);
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        if (dir == 0) DPx[k][threadIdx.y][threadIdx.x + 1] = Dp[k];
+        else DPy[k][threadIdx.y + 1][threadIdx.x] = Dp[k];
+      }
+    }
+  }
+  // faces on the low edges of the tile: y-faces below row 0 (threads 0..31), x-faces left of
+  // column 0 (threads 32..39)
+  if (tid < PTX + PTY) {
+    const int dir = (tid < PTX) ? 1 : 0;
+    const int cx = (dir == 1) ? tid : -1, cy = (dir == 1) ? -1 : tid - PTX;  // tile cell on the low side
+    if (i0 + max(cx, 0) < G.nx && j0 + max(cy, 0) < G.ny) {
+      double sl[4], Dm[3], Dp[3];
+      hi_face(T, cx + PH, cy + PH, dir, order, eps_dry, g, sl, Dm, Dp);
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        if (dir == 0) DPx[k][cy][0] = Dp[k];
+        else DPy[k][0][cx] = Dp[k];
+      }
+    }
+  }
+  __syncthreads();
+  if (!active) return;
   const double dt = sc->dt;
   double dU[2][3];  // per direction: (h, normal q, tangential q)
 #pragma unroll
   for (int dir = 0; dir < 2; ++dir) {
-    int di = (dir == 0), dj = (dir == 1);
     Prim Pc = get_prim(T, lx, ly, dir);
-    Prim Pm = get_prim(T, lx - di, ly - dj, dir);
-    Prim Pp = get_prim(T, lx + di, ly + dj, dir);
-    double sc_[4], sm[4], sp[4];
-    cell_slopes(T, lx, ly, dir, order, eps_dry, sc_);
-    cell_slopes(T, lx - di, ly - dj, dir, order, eps_dry, sm);
-    cell_slopes(T, lx + di, ly + dj, dir, order, eps_dry, sp);
-    // S3 face states.  "hi" face (i+1/2): left = c + s/2, right = p - s/2
-    double hL = Pc.h + 0.5 * sc_[1], eL = Pc.eta + 0.5 * sc_[0];
-    double uL = Pc.un + 0.5 * sc_[2], vL = Pc.ut + 0.5 * sc_[3];
-    double hR = Pp.h - 0.5 * sp[1], eR = Pp.eta - 0.5 * sp[0];
-    double uR = Pp.un - 0.5 * sp[2], vR = Pp.ut - 0.5 * sp[3];
-    double Dm_hi[3], Dp_hi[3];
-    face_fluct(g, hL, eL, uL, vL, hR, eR, uR, vR, Dm_hi, Dp_hi);
-    // "lo" face (i-1/2): left = m + s/2, right = c - s/2
-    double hl = Pm.h + 0.5 * sm[1], el = Pm.eta + 0.5 * sm[0];
-    double ul = Pm.un + 0.5 * sm[2], vl = Pm.ut + 0.5 * sm[3];
-    double hr = Pc.h - 0.5 * sc_[1], er = Pc.eta - 0.5 * sc_[0];
-    double ur = Pc.un - 0.5 * sc_[2], vr = Pc.ut - 0.5 * sc_[3];
-    double Dm_lo[3], Dp_lo[3];
-    face_fluct(g, hl, el, ul, vl, hr, er, ur, vr, Dm_lo, Dp_lo);
+    const double* s_ = sown[dir];
+    // own face states: "hi" face left state = c + s/2, "lo" face right state = c - s/2
+    double hL = Pc.h + 0.5 * s_[1], uL = Pc.un + 0.5 * s_[2], vL = Pc.ut + 0.5 * s_[3];
+    double hr = Pc.h - 0.5 * s_[1], ur = Pc.un - 0.5 * s_[2], vr = Pc.ut - 0.5 * s_[3];
     // in-cell term I_i of (22) = F_c(U^-_{i+1/2}) - F_c(U^+_{i-1/2}) + g h_i sigma_eta e2 (S5)
     double qnL = hL * uL, qnr = hr * ur;
     double Fhi[3] = {qnL, qnL * uL, qnL * vL};
     double Flo[3] = {qnr, qnr * ur, qnr * vr};
 #pragma unroll
-    for (int k = 0; k < 3; ++k) dU[dir][k] = Dm_hi[k] + Dp_lo[k] + (Fhi[k] - Flo[k]);
-    dU[dir][1] += g * Pc.h * sc_[0];
+    for (int k = 0; k < 3; ++k) {
+      double Dp_lo = (dir == 0) ? DPx[k][threadIdx.y][threadIdx.x] : DPy[k][threadIdx.y][threadIdx.x];
+      dU[dir][k] = Dm_hi[dir][k] + Dp_lo + (Fhi[k] - Flo[k]);
+    }
+    dU[dir][1] += g * Pc.h * s_[0];
   }
   size_t k = (size_t)j * G.nx + i;
   double lxr = dt / G.dx, lyr = dt / G.dy;
