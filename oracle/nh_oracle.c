@@ -787,6 +787,60 @@ static void relaxation(nho_ctx* c, double* h, double* qx, double* qy, double* w,
     }
 }
 
+/* S11b: absorbing relaxation zones (L415-440): the relaxation of S11 with the target
+ * U* = w* = p* = 0, read as eta* = 0, q* = 0 (h* = max(H, 0); "U* = 0" would drain the basin, R18).
+ * Reading R29: width L on a side, k_Rel = ceil(L / dx) cells; m = sqrt(1 - (d/L)^2) with d measured
+ * from the inner end of the zone (R18), m = 1 outside; node values use the mean of the two
+ * adjacent cell coefficients (0 beyond the boundary, L429); the update is written
+ * a <- a + (1 - m)(a* - a) so that a state already at the target is left bit-identical (lake at
+ * rest); sides are applied in the order x-lo, x-hi, y-lo, y-hi (corners take both factors). */
+static double absorb_m(double L, double dxy, int idx_from_boundary) {
+  double x = ((double)idx_from_boundary + 0.5) * dxy;
+  double d = L - x;
+  if (d <= 0.0) return 1.0;
+  if (d >= L) return 0.0;
+  return sqrt(1.0 - (d / L) * (d / L));
+}
+static void absorb_side(nho_ctx* c, int side, double L, double* h, double* qx, double* qy, double* w,
+                        double* p) {
+  const int xdir = (side < 2), hi = (side & 1);
+  const int n = xdir ? c->nx : c->ny, nn = xdir ? c->nnx : c->nny;
+  const double dxy = xdir ? c->dx : c->dy;
+  int krel = (int)ceil(L / dxy);
+  if (krel > n) krel = n;
+  const int nother = xdir ? c->ny : c->nx, nnother = xdir ? c->nny : c->nnx;
+#pragma omp parallel for if (nother >= 48) schedule(static)
+  for (int t = 0; t < nother; ++t)
+    for (int s = 0; s < krel; ++s) {          /* s = cell index counted from the boundary */
+      int a = hi ? n - 1 - s : s;
+      size_t k = xdir ? CIDX(c, a, t) : CIDX(c, t, a);
+      double f = 1.0 - absorb_m(L, dxy, s);
+      double hs = fmax(c->H[k], 0.0);
+      h[k] = h[k] + f * (hs - h[k]);
+      qx[k] = qx[k] + f * (0.0 - qx[k]);
+      qy[k] = qy[k] + f * (0.0 - qy[k]);
+    }
+#pragma omp parallel for if (nnother >= 48) schedule(static)
+  for (int t = 0; t < nnother; ++t)
+    for (int s = 0; s <= krel; ++s) {         /* s = node line counted from the boundary line */
+      int a = hi ? n - s : s;                  /* node line index in the (n+1)-line numbering */
+      if (nn == n) {                           /* periodic direction never has zones */
+        continue;
+      }
+      double mo = (s - 1 >= 0) ? absorb_m(L, dxy, s - 1) : 0.0;   /* cell towards the boundary */
+      double mi = (s < n) ? absorb_m(L, dxy, s) : 1.0;            /* cell towards the interior */
+      double f = 1.0 - 0.5 * (mo + mi);
+      size_t k = xdir ? NIDX(c, a, t) : NIDX(c, t, a);
+      w[k] = w[k] + f * (0.0 - w[k]);
+      p[k] = p[k] + f * (0.0 - p[k]);
+    }
+}
+static void absorbing_zones(nho_ctx* c, double* h, double* qx, double* qy, double* w, double* p) {
+  const double L[4] = { c->prm.abs_xlo, c->prm.abs_xhi, c->prm.abs_ylo, c->prm.abs_yhi };
+  for (int side = 0; side < 4; ++side)
+    if (L[side] > 0.0) absorb_side(c, side, L[side], h, qx, qy, w, p);
+}
+
 /* S6-S10 on U* = (h1,qx1,qy1) with w_in; results to (qx_out,qy_out,w_out), p in c->p. */
 static int nonhydro_part(nho_ctx* c, const double* w_in, double dt, double* qx_out, double* qy_out,
                          double* w_out) {
@@ -832,6 +886,7 @@ static int stage(nho_ctx* c, double dt, double t0) {
     memcpy(c->qy, c->qy1, nc * sizeof(double));
   }
   if (c->prm.gen_on) relaxation(c, c->h, c->qx, c->qy, c->w, c->p, t0 + dt);
+  absorbing_zones(c, c->h, c->qx, c->qy, c->w, c->p);
   return st;
 }
 
@@ -864,6 +919,10 @@ int nho_create(nho_ctx** out, int nx, int ny, double dx, double dy, const double
   if (!(prm->manning_n >= 0.0)) return NHO_EINVAL;
   if (prm->solver != 0 && prm->solver != 1) return NHO_EINVAL;
   if (!(prm->srj_rel >= 0.0)) return NHO_EINVAL;
+  if (!(prm->abs_xlo >= 0.0) || !(prm->abs_xhi >= 0.0) || !(prm->abs_ylo >= 0.0) || !(prm->abs_yhi >= 0.0)) return NHO_EINVAL;
+  if ((prm->abs_xlo > 0.0 || prm->abs_xhi > 0.0) && prm->bc_xlo == NHO_BC_PERIODIC) return NHO_EINVAL;
+  if ((prm->abs_ylo > 0.0 || prm->abs_yhi > 0.0) && prm->bc_ylo == NHO_BC_PERIODIC) return NHO_EINVAL;
+  if (prm->abs_xlo > 0.0 && prm->gen_on) return NHO_EINVAL;   /* the generating zone owns x-lo */
   if (prm->solver == 1 && (!(prm->srj_eps > 0.0) || prm->srj_mmax < 1 || prm->srj_mmax > 4096 ||
                            (prm->srj_mmax & (prm->srj_mmax - 1)) != 0)) return NHO_EINVAL;
   if (prm->breaking && !(prm->B1 > 0.0 && prm->B2 > 0.0)) return NHO_EINVAL;

@@ -37,6 +37,8 @@ typedef struct {
   double manning_n;    /* Gauckler-Manning coefficient n (L61-65, L773-775); 0 = frictionless     */
   double srj_eps;      /* solver 1: stop when the Jacobi increment of (32) is < srj_eps (L507-514) */
   double srj_rel;      /* solver 1: if > 0 the tolerance of (32) is srj_rel * max|b/A_C| instead    */
+  double abs_xlo, abs_xhi, abs_ylo, abs_yhi; /* widths L_Rel of absorbing relaxation zones on the
+                          four sides (L415-440; R18, R29); 0 = none                                */
   int breaking;        /* 1: eddy-viscosity breaking sources on (section 3)             */
   int nonhydro;        /* 0: hydrostatic SWE path only (p = 0, w frozen)                */
   int time_order;      /* 1 or 2 (TVD RK2, L406, L516)                                  */

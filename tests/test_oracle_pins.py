@@ -764,3 +764,77 @@ def test_srj_relative_rule_bounds_the_scaled_residual(O):
     bmax = np.max(np.abs(b.ravel() / D))
     assert it > 3 and np.max(np.abs(z)) < 1e-8 * bmax * (1 + 1e-6)
     assert abs(E - np.max(np.abs(z))) <= 1e-3 * E
+
+
+# ---------------------------------------------------------------- absorbing relaxation zones
+# (readings R18, R29)
+def test_absorbing_zone_closed_form_on_a_uniform_state(O):
+    # A uniform current over a flat bottom is a fixed point of the finite-volume step, so one
+    # first-order step leaves exactly the relaxation U~ = m U + (1 - m) U* of L425 with
+    # m = sqrt(1 - (d/L)^2) (L429), d from the inner end of the zone (R18), U* = (H, 0, 0).
+    nx, ny, dx, h0, a, q0, L = 40, 6, 0.5, 2.0, 0.25, 0.7, 4.2
+    H = np.full((ny, nx), h0)
+    o = O.Oracle(nx, ny, dx, dx, H, nonhydro=0, time_order=1, abs_xlo=L, bc_ylo=PER, bc_yhi=PER)
+    o.set_state(H + a, np.full((ny, nx), q0), np.zeros((ny, nx)))
+    o.step(1)
+    s = o.get_state()
+    x = (np.arange(nx) + 0.5) * dx
+    d = np.clip(L - x, 0.0, L)
+    m = np.sqrt(1.0 - (d / L) ** 2)
+    assert 0 < int(np.sum(m < 1.0)) <= int(np.ceil(L / dx))     # inside the k_Rel cells of L423
+    np.testing.assert_allclose(s["h"][2] - h0, m * a, rtol=0, atol=1e-15)
+    np.testing.assert_allclose(s["qx"][2], m * q0, rtol=0, atol=1e-15)
+    assert np.all(s["h"][:, m == 1.0] == h0 + a) and np.all(s["qx"][:, m == 1.0] == q0)
+
+
+def test_absorbing_zones_keep_rest_exactly_and_act_only_inside_the_zones(O):
+    cfg = inputs.make_config(2, nx=64, ny=48)
+    zones = dict(abs_xlo=6.0, abs_xhi=9.5, abs_ylo=4.0, abs_yhi=7.0)
+    o = make(O, cfg, **zones)
+    o.step(5)
+    s = o.get_state()
+    assert np.max(np.abs(s["qx"])) == 0.0 and np.max(np.abs(s["qy"])) == 0.0
+    assert np.max(np.abs(s["h"] - cfg["h"])) <= 1e-13 * 5.0
+    # a moving state: one first-order stage with and without zones differs only inside the zones
+    st = inputs.random_smooth_state(64, 48, 1.0, 1.0, seed=8, depth=2.0)
+    outs = []
+    for kw in ({}, zones):
+        o = O.Oracle(64, 48, 1.0, 1.0, st["H"], time_order=1, **kw)
+        o.set_state(st["h"], st["qx"], st["qy"], st["w"], st["p"])
+        o.step(1)
+        outs.append(o.get_state())
+    ins = (slice(4, 48 - 7), slice(6, 64 - 10))         # cells beyond ceil(L/dx) of every side
+    for k in ("h", "qx", "qy"):
+        assert np.array_equal(outs[0][k][ins], outs[1][k][ins]), k
+        assert not np.array_equal(outs[0][k], outs[1][k])
+    insn = (slice(5, 49 - 8), slice(7, 65 - 11))
+    for k in ("w", "p"):
+        assert np.array_equal(outs[0][k][insn], outs[1][k][insn]), k
+        assert not np.array_equal(outs[0][k], outs[1][k])
+
+
+def test_absorbing_zone_removes_the_reflection_from_a_wall(O):
+    nx, ny, dx, h0 = 400, 4, 0.25, 1.0
+    H = np.full((ny, nx), h0)
+    x = (np.arange(nx) + 0.5) * dx
+    eta = 0.02 * np.exp(-((x - 60.0) / 3.0) ** 2)
+    c0 = np.sqrt(9.81 * h0)
+    res = {}
+    for L in (0.0, 25.0):
+        o = O.Oracle(nx, ny, dx, dx, H, bc_xlo=OUT, bc_xhi=WALL, bc_ylo=PER, bc_yhi=PER, abs_xhi=L,
+                     nonhydro=0)   # the zone acts on the hydrostatic and the full step alike
+        o.set_state(H + eta[None, :], np.tile(c0 * eta, (ny, 1)), np.zeros((ny, nx)))
+        while o.info().t < 26.0:       # right-going pulse: reaches the wall at t ~ 13, back at x ~ 60 at t ~ 26
+            o.step(20)
+        s = o.get_state()
+        res[L] = np.max(np.abs(s["h"][1, :300] - h0))
+    assert res[0.0] > 0.005            # the wall reflects the pulse back into the interior
+    assert res[25.0] < 0.1 * res[0.0]  # the zone (about 2.5 pulse widths, L <= L_Rel <= 1.5 L) absorbs it
+
+
+def test_absorbing_zone_parameters_are_validated(O):
+    H = np.ones((8, 8))
+    for bad in (dict(abs_xlo=-1.0), dict(abs_ylo=2.0, bc_ylo=PER, bc_yhi=PER),
+                dict(abs_xlo=2.0, gen_on=1, gen_A=0.1, gen_h0=1.0, gen_Lrel=2.0)):
+        with pytest.raises(O.OracleError):
+            O.Oracle(8, 8, 1.0, 1.0, H, **bad)
