@@ -61,6 +61,9 @@ typedef struct {
   double manning_n;   /* Gauckler-Manning n (L61-65, L773-775), semi-implicit (R27); default 0 = off */
   double srj_eps;     /* solver 1: stop when the Jacobi increment of eq. (32) is < srj_eps; 1e-5  */
   double srj_rel;     /* solver 1: if > 0, the tolerance of (32) is srj_rel * max|b / A_C| instead */
+  double abs_xlo, abs_xhi, abs_ylo, abs_yhi; /* widths L_Rel of the absorbing relaxation zones on
+                         the four sides (L415-440; R18, R29); 0 = none (default).  Not on
+                         a periodic side; abs_xlo not together with gen_on: NH_EINVAL           */
   int breaking;       /* 1: eddy-viscosity breaking sources on (section 3, eqs (8)-(12))    */
   int nonhydro;       /* 0: hydrostatic SWE path only (p = 0, w frozen); default 1          */
   int time_order;     /* 1, or 2 = two-stage TVD Runge-Kutta (L406, L516, L544); default 2  */

@@ -178,7 +178,10 @@ void nonhydro_part(nh_ctx* c, const double* h1, const double* qx1, const double*
 }
 
 // w changes within a stage only through the correction (nonhydro) or the relaxation zone
-inline bool w_moves(const nh_ctx* c) { return c->prm.nonhydro || c->prm.gen_on; }
+inline bool absorbing(const nh_ctx* c) {
+  return c->prm.abs_xlo > 0.0 || c->prm.abs_xhi > 0.0 || c->prm.abs_ylo > 0.0 || c->prm.abs_yhi > 0.0;
+}
+inline bool w_moves(const nh_ctx* c) { return c->prm.nonhydro || c->prm.gen_on || absorbing(c); }
 
 // one stage Phi_dt: cell slot `in` -> `out`, node slot `inw` -> `outw` (== inw when w does not
 // move); stage_idx selects the relaxation clock (end time of the stage).
@@ -197,6 +200,7 @@ void stage(nh_ctx* c, int in, int inw, int out, int outw, int stage_idx) {
   }
   if (c->prm.gen_on)
     nh_launch_relax(c, c->h[out], c->qx[out], c->qy[out], c->w[outw], c->p, stage_idx);
+  if (absorbing(c)) nh_launch_absorb(c, c->h[out], c->qx[out], c->qy[out], c->w[outw], c->p);
 }
 
 void ensure_lambda(nh_ctx* c) {
@@ -234,6 +238,10 @@ int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* 
   if (!(prm->manning_n >= 0.0)) return NH_EINVAL;
   if (prm->solver != 0 && prm->solver != 1) return NH_EINVAL;
   if (!(prm->srj_rel >= 0.0)) return NH_EINVAL;
+  if (!(prm->abs_xlo >= 0.0) || !(prm->abs_xhi >= 0.0) || !(prm->abs_ylo >= 0.0) || !(prm->abs_yhi >= 0.0)) return NH_EINVAL;
+  if ((prm->abs_xlo > 0.0 || prm->abs_xhi > 0.0) && prm->bc_xlo == NH_BC_PERIODIC) return NH_EINVAL;
+  if ((prm->abs_ylo > 0.0 || prm->abs_yhi > 0.0) && prm->bc_ylo == NH_BC_PERIODIC) return NH_EINVAL;
+  if (prm->abs_xlo > 0.0 && prm->gen_on) return NH_EINVAL;  // the generating zone owns x-lo
   if (prm->solver == 1 && (!(prm->srj_eps > 0.0) || prm->srj_mmax < 1 || prm->srj_mmax > 4096 ||
                            (prm->srj_mmax & (prm->srj_mmax - 1)) != 0)) return NH_EINVAL;
   if (prm->breaking && !(prm->B1 > 0.0 && prm->B2 > 0.0)) return NH_EINVAL;

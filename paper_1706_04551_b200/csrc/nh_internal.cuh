@@ -185,6 +185,7 @@ void nh_launch_correct(nh_ctx* c, const double* h, const double* z, const double
                        const double* qy2, const double* w2, const double* p, double* qx_out,
                        double* qy_out, double* w_out);
 void nh_launch_relax(nh_ctx* c, double* h, double* qx, double* qy, double* w, double* p, int stage);
+void nh_launch_absorb(nh_ctx* c, double* h, double* qx, double* qy, double* w, double* p);
 void nh_launch_nodes_out(nh_ctx* c, const double* src, double* dst);
 // nh_solver.cu
 int nh_solver_setup(nh_ctx* c);  // occupancy -> cooperative grid, partial buffer

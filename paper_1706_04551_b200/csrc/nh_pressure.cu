@@ -414,6 +414,52 @@ k_relax(NhGrid G, const NhScal* sc, int stage, double g, double A, double h0, do
   }
 }
 
+// S11b: absorbing relaxation zone on one side (L415-440; R18, R29): the relaxation of S11 towards
+// eta* = 0, q* = w* = p* = 0, a <- a + (1 - m)(a* - a), m = sqrt(1 - (d/L)^2), d from the inner end
+// of the zone; node coefficients are the mean of the two adjacent cell coefficients (0 beyond the
+// boundary).  side: 0 x-lo, 1 x-hi, 2 y-lo, 3 y-hi; s = distance from the boundary in cells / lines.
+__device__ __forceinline__ double absorb_m(double L, double dxy, int s) {
+  double x = ((double)s + 0.5) * dxy;
+  double d = L - x;
+  if (d <= 0.0) return 1.0;
+  if (d >= L) return 0.0;
+  return sqrt(1.0 - (d / L) * (d / L));
+}
+__global__ void __launch_bounds__(256)
+k_absorb(NhGrid G, int side, double L, int krel, const double* __restrict__ H,
+         double* __restrict__ h, double* __restrict__ qx, double* __restrict__ qy,
+         double* __restrict__ w, double* __restrict__ p) {
+  const bool xdir = side < 2, hi = side & 1;
+  const int n = xdir ? G.nx : G.ny;
+  const double dxy = xdir ? G.dx : G.dy;
+  const int nother = xdir ? G.ny : G.nx;  // both zone directions are non-periodic: n + 1 node lines
+  const int nnother = xdir ? G.nny : G.nnx;
+  const int ns = krel + 1;
+  size_t tot = (size_t)ns * (nother + 1);
+  for (size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x; e < tot;
+       e += (size_t)gridDim.x * blockDim.x) {
+    int s = (int)(e % ns), t = (int)(e / ns);
+    if (s < krel && t < nother) {
+      int a = hi ? n - 1 - s : s;
+      size_t k = xdir ? (size_t)t * G.nx + a : (size_t)a * G.nx + t;
+      double f = 1.0 - absorb_m(L, dxy, s);
+      double hs = fmax(H[k], 0.0);
+      h[k] = h[k] + f * (hs - h[k]);
+      qx[k] = qx[k] + f * (0.0 - qx[k]);
+      qy[k] = qy[k] + f * (0.0 - qy[k]);
+    }
+    if (t < nnother) {
+      int a = hi ? n - s : s;
+      double mo = (s - 1 >= 0) ? absorb_m(L, dxy, s - 1) : 0.0;
+      double mi = (s < n) ? absorb_m(L, dxy, s) : 1.0;
+      double f = 1.0 - 0.5 * (mo + mi);
+      size_t k = xdir ? (size_t)t * G.np + a : (size_t)a * G.np + t;
+      w[k] = w[k] + f * (0.0 - w[k]);
+      p[k] = p[k] + f * (0.0 - p[k]);
+    }
+  }
+}
+
 // internal plane -> dense public node layout: fill the duplicate lines of periodic directions
 __global__ void __launch_bounds__(BX* BY)
 k_nodes_out(NhGrid G, const double* __restrict__ src, double* __restrict__ dst) {
@@ -495,6 +541,20 @@ void nh_launch_relax(nh_ctx* c, double* h, double* qx, double* qy, double* w, do
                                                        P.gen_x0, P.gen_Lrel, krel, c->H, h, qx, qy,
                                                        w, p);
   c->launches++;
+}
+void nh_launch_absorb(nh_ctx* c, double* h, double* qx, double* qy, double* w, double* p) {
+  const double L[4] = {c->prm.abs_xlo, c->prm.abs_xhi, c->prm.abs_ylo, c->prm.abs_yhi};
+  for (int side = 0; side < 4; ++side) {
+    if (!(L[side] > 0.0)) continue;
+    const bool xdir = side < 2;
+    const int n = xdir ? c->g.nx : c->g.ny, nother = xdir ? c->g.ny : c->g.nx;
+    int krel = (int)ceil(L[side] / (xdir ? c->g.dx : c->g.dy));
+    if (krel > n) krel = n;
+    size_t tot = (size_t)(krel + 1) * (nother + 1);
+    k_absorb<<<grid_1d(c, tot, 256), 256, 0, c->stream>>>(c->g, side, L[side], krel, c->H, h, qx, qy,
+                                                          w, p);
+    c->launches++;
+  }
 }
 void nh_launch_nodes_out(nh_ctx* c, const double* src, double* dst) {
   k_nodes_out<<<grid2(c->g.nx + 1, c->g.ny + 1), dim3(BX, BY), 0, c->stream>>>(c->g, src, dst);

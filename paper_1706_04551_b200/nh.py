@@ -30,6 +30,7 @@ class Params(C.Structure):
         ("B1", C.c_double), ("B2", C.c_double), ("solver_rtol", C.c_double),
         ("gen_A", C.c_double), ("gen_h0", C.c_double), ("gen_x0", C.c_double), ("gen_Lrel", C.c_double),
         ("manning_n", C.c_double), ("srj_eps", C.c_double), ("srj_rel", C.c_double),
+        ("abs_xlo", C.c_double), ("abs_xhi", C.c_double), ("abs_ylo", C.c_double), ("abs_yhi", C.c_double),
         ("breaking", C.c_int), ("nonhydro", C.c_int), ("time_order", C.c_int), ("space_order", C.c_int),
         ("bc_xlo", C.c_int), ("bc_xhi", C.c_int), ("bc_ylo", C.c_int), ("bc_yhi", C.c_int),
         ("solver_maxit", C.c_int), ("gen_on", C.c_int), ("precision", C.c_int), ("solver", C.c_int),

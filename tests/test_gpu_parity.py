@@ -473,3 +473,39 @@ def test_srj_relative_tolerance_bit_exact(O, G):
     _, g2 = both(O, G, cfg, srj_rel=1e-12)
     g2.step(2)
     assert g2.sync() == 0 and g2.info().iters_total > g.info().iters_total
+
+
+# ---------------------------------------------------------------- absorbing relaxation zones (R29)
+@pytest.mark.parametrize("nonhydro", [0, 1])
+def test_absorbing_zones_parity(O, G, nonhydro):
+    zones = dict(abs_xlo=1.3, abs_xhi=2.0, abs_ylo=0.9, abs_yhi=1.55)
+    cfg = rnd_cfg(72, 51, (OUT, WALL, OUT, OUT), seed=61, dry=0.15, dx=0.2, dy=0.25, nonhydro=nonhydro,
+                  solver=1, srj_eps=1e-11, **zones)
+    o, g = both(O, G, cfg)
+    o.step(4)
+    g.step(4)
+    assert g.sync() == 0
+    so, sg = o.get_state(), g.get_state()
+    for k in so:                       # solver 1: the whole step is bit-exact, zones included
+        assert np.array_equal(so[k], sg[k]), k
+    _, gb = both(O, G, cfg, solver=0)  # and with the default solver within the tolerances
+    ob, _ = both(O, G, cfg, solver=0)
+    ob.step(4)
+    gb.step(4)
+    assert gb.sync() == 0
+    assert_parity(gb.get_state(), ob.get_state(), cfg["H"], cfg["h0"])
+
+
+def test_absorbing_zones_radial_hump_reduced(O, G):
+    # config 3 with absorbing zones of one hump width on all four open sides
+    cfg = inputs.make_config(3, nx=160, ny=128)
+    zones = dict(abs_xlo=1.0, abs_xhi=1.0, abs_ylo=1.0, abs_yhi=1.0)
+    o, g = both(O, G, cfg, **zones)
+    o.step(12)
+    g.step(12)
+    assert g.sync() == 0
+    assert_parity(g.get_state(), o.get_state(), cfg["H"], cfg["h0"])
+    for bad in (dict(abs_xhi=-0.5), dict(abs_ylo=1.0, bc_ylo=PER, bc_yhi=PER),
+                dict(abs_xlo=1.0, gen_on=1, gen_A=0.1, gen_h0=0.5, gen_Lrel=1.0)):
+        with pytest.raises(G.NHError):
+            G.NH(16, 16, 0.1, 0.1, np.full((16, 16), 0.5), **bad)
