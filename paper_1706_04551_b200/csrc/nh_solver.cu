@@ -216,6 +216,10 @@ __device__ __forceinline__ double2 stencil2(const RowC& C, double2 m, double2 c,
 // live rows spill at 128 registers; 2271 with 192-thread CTAs and 168 registers)).
 constexpr bool PF_B = true;    // pass B: request the next step's operands before computing this one
 constexpr bool PF_CA = false;  // pass CA: all ten operand loads of a step up front, then compute
+#ifndef NH_DEFER_CA
+#define NH_DEFER_CA 1
+#endif
+constexpr bool DEFER_CA = NH_DEFER_CA;  // pass CA: next step's loads issued before this step's stores
 
 // pass B: s = r - alpha v (rows Ja-1..Jb), t = (A M^-1) s (rows Ja..Jb-1);
 // partials: t.s, t.t, s.s, r0.s, r0.t
@@ -349,11 +353,43 @@ __device__ __forceinline__ void pass_CA(const SolveP& P, double alpha, double om
       if (U.own1) acc[0] = fma(cur.C.q.y, vv.y, acc[0]);
       pm = pc; pc = pn;
     };
-    RowCA A, B;
-    if (PF_CA) ld_set(A, U.Ja + 1, U.Ja);
-    for (int j = U.Ja; j < U.Jb; j += 2) {  // ping-pong operand sets: no register rotation
-      step(j, A, B);
-      if (j + 1 < U.Jb) step(j + 1, B, A);
+    if (!FIRST && DEFER_CA) {
+      // One operand set; the loads of step j+1 are issued as soon as step j has consumed its
+      // operands, BEFORE its four stores (ghost-image logic included) and its dot-product terms,
+      // which then run in the shadow of the memory latency.
+      RowCA X;
+      ld_set(X, U.Ja + 1, U.Ja);
+      for (int j = U.Ja; j < U.Jb; ++j) {
+        const RowV& V = X.V;
+        const bool own_next = j + 1 < U.Jb;
+        double2 sv = make_double2(fma(-alpha, V.v.x, V.r.x), fma(-alpha, V.v.y, V.r.y));
+        double2 rn = make_double2(fma(-omega, V.t.x, sv.x), fma(-omega, V.t.y, sv.y));
+        double2 pn = make_double2(fma(beta, fma(-omega, V.v.x, V.p.x), rn.x),
+                                  fma(beta, fma(-omega, V.v.y, V.p.y), rn.y));
+        double2 yy = make_double2(V.y.x + fma(omega, sv.x, alpha * V.p.x),
+                                  V.y.y + fma(omega, sv.y, alpha * V.p.y));
+        double2 vv = stencil2(X.C, pm, pc, pn);
+        const double2 q = X.C.q;
+        if (own_next) ld_set(X, min(j + 2, U.Jb), j + 1);  // operands of the next step
+        if (own_next) {
+          st2(P.y, P, U, j + 1, yy);
+          st2(rN, P, U, j + 1, rn);
+          st2(pN, P, U, j + 1, pn);
+          if (U.own0) acc[1] = fma(rn.x, rn.x, acc[1]);
+          if (U.own1) acc[1] = fma(rn.y, rn.y, acc[1]);
+        }
+        st2(vN, P, U, j, vv);
+        if (U.own0) acc[0] = fma(q.x, vv.x, acc[0]);
+        if (U.own1) acc[0] = fma(q.y, vv.y, acc[0]);
+        pm = pc; pc = pn;
+      }
+    } else {
+      RowCA A, B;
+      if (PF_CA) ld_set(A, U.Ja + 1, U.Ja);
+      for (int j = U.Ja; j < U.Jb; j += 2) {  // ping-pong operand sets: no register rotation
+        step(j, A, B);
+        if (j + 1 < U.Jb) step(j + 1, B, A);
+      }
     }
   }
   block_partials<2>(acc, P.part, buf, red);
