@@ -97,6 +97,18 @@ class ClockSampler:
             os.unlink(self.path)
         except Exception:
             pass
+        if not sm:   # timed region shorter than one sampling period: one reading right after it
+            try:
+                r = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                    "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=20)
+                f = [x.strip() for x in r.stdout.strip().splitlines()[0].split(",")]
+                sm.append(float(f[0])); mx.append(float(f[1]))
+                for n, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+                out["note"] = "timed region < 200 ms: sampled once right after it"
+            except Exception:
+                pass
         if sm:
             out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), samples=len(sm))
         out["reasons"] = sorted(reasons)

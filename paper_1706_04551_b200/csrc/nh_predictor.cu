@@ -122,7 +122,10 @@ __device__ __forceinline__ void hi_face(const PredTile& T, int lx, int ly, int d
 // own update and publishes D^+ for its neighbour through shared memory; the faces on the low
 // edges of the tile (32 in y, 8 in x) are solved by the first 40 threads.  (The first version had
 // every cell solve its four faces and limit five cells: 2400 instructions per cell.)
-__global__ void __launch_bounds__(PTX* PTY)
+#ifndef NH_PRED_MINB
+#define NH_PRED_MINB 4  // 64 registers: 10.3 ms per two launches at 8192^2 (2: 15.7, 3: 11.9, 5: 10.2, 6: 12.4)
+#endif
+__global__ void __launch_bounds__(PTX* PTY, NH_PRED_MINB)
 k_predictor(NhGrid G, double g, double delta, double eps_dry, double manning_n, int order,
             const NhScal* sc, const double* __restrict__ H, const double* __restrict__ h,
             const double* __restrict__ qx, const double* __restrict__ qy,
