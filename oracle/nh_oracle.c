@@ -585,14 +585,14 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
       for (int I = 0; I < nnx; ++I) x[NIDX(c, I, J)] = 0.0;
     return NHO_OK;
   }
-  if (!(rho < 1.0)) {
-    snprintf(c->err, sizeof(c->err), "srj: matrix not strictly diagonally dominant (rho = %g)", rho);
-    return NHO_ENOCONV;
-  }
-  /* cycle length and schedule */
-  const double gap = sqrt(2.0 * (1.0 - rho));
+  /* cycle length and schedule.  Where a row is not strictly diagonally dominant (rho >= 1: the
+   * Gershgorin interval reaches 0, e.g. across a discontinuous free surface) there is no interval to
+   * place Chebyshev nodes on: the method falls back to the plain Jacobi method (one factor, 1). */
+  const int dominant = (rho < 1.0);
+  const double gap = dominant ? sqrt(2.0 * (1.0 - rho)) : 0.0;
   int M = 1;
-  while (M < c->prm.srj_mmax && (double)M * gap < 7.6) M *= 2;
+  if (dominant)
+    while (M < c->prm.srj_mmax && (double)M * gap < 7.6) M *= 2;
   int* perm = (int*)malloc(sizeof(int) * (size_t)M);
   double* omega = (double*)malloc(sizeof(double) * (size_t)M);
   if (!perm || !omega) { free(perm); free(omega); return NHO_ENOMEM; }
@@ -604,7 +604,7 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
     }
   for (int i = 0; i < M; ++i) {
     double cosv = cos(3.14159265358979323846 * (double)(2 * perm[i] - 1) / (double)(2 * M));
-    omega[i] = 1.0 / (1.0 - rho * cosv);
+    omega[i] = dominant ? 1.0 / (1.0 - rho * cosv) : 1.0;
   }
   int iters = 0, status = NHO_OK;
   double E = 0.0;

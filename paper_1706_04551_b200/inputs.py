@@ -167,6 +167,22 @@ def config5_tsunami(nx=8192, ny=8192, dx=100.0, steps=200, seed=SEEDS[5], nmodes
     return _pack("tsunami_basin", nx, ny, dx, dx, H, h, 0.0, 0.0, params, 4000.0, steps)
 
 
+def paper_dam_break(n=250):
+    """The paper's own timing workload (section 7.7, Table 2): circular dam break
+    on [-5,5]^2, H = 1 - 0.25 exp(-x^2 - y^2), h0 = H inside r <= 0.5 and H + 0.25 outside, q = 0,
+    CFL 0.9, open boundaries, run to t = 1; n x n cells (the paper: 250 ... 1500).  The initial
+    condition is the paper's formula, not a dataset.  `steps` is a rough count (the run is to t=1)."""
+    dx = 10.0 / n
+    x = (np.arange(n) + 0.5) * dx - 5.0
+    X, Y = np.meshgrid(x, x)
+    r2 = X * X + Y * Y
+    H = 1.0 - 0.25 * np.exp(-r2)
+    h = np.where(np.sqrt(r2) <= 0.5, H, H + 0.25)
+    params = dict(g=9.81, cfl=0.9, nonhydro=1, breaking=0, time_order=2,
+                  bc_xlo=BC_OUTFLOW, bc_xhi=BC_OUTFLOW, bc_ylo=BC_OUTFLOW, bc_yhi=BC_OUTFLOW)
+    return _pack("paper_dam_break", n, n, dx, dx, H, h, 0.0, 0.0, params, 1.25, int(0.8 * n))
+
+
 CONFIGS = {1: config1_channel, 2: config2_lake, 3: config3_radial, 4: config4_beach,
            5: config5_tsunami}
 
