@@ -323,6 +323,50 @@ def run_b200(args):
     return 0
 
 
+def run_table2(args):
+    """The paper's own timing experiment (Table 2) on this GPU: circular dam
+    break to t = 1, CFL 0.9, SWE (nonhydro = 0) and NH with the paper's solver (solver 1) at its
+    three tolerances, wall time of the whole time loop on the device (CUDA events around it; whole
+    steps until t >= 1, checked on the host every 25 steps).  Context, not the headline metric."""
+    import torch
+    from paper_1706_04551_b200 import inputs, nh
+    torch.cuda.set_device(0)
+    sizes = [int(x) for x in args.table2.split(",")]
+    rows = []
+    for n in sizes:
+        cfg = inputs.paper_dam_break(n)
+        row = {"n": n}
+        for tag, over in (("swe", dict(nonhydro=0)), ("nh_1e-3", dict(solver=1, srj_eps=1e-3)),
+                          ("nh_1e-4", dict(solver=1, srj_eps=1e-4)), ("nh_1e-5", dict(solver=1, srj_eps=1e-5))):
+            prm = dict(cfg["params"]); prm.update(over)
+            prm["solver_maxit"] = 1000000   # plain-Jacobi phases across the initial discontinuity are long
+            stream = torch.cuda.Stream()
+            sim = nh.NH(n, n, cfg["dx"], cfg["dy"], cfg["H"], stream=stream, **prm)
+            sim.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
+            sim.step(2); sim.sync()                                   # warm-up (module load, caches)
+            sim.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            i0 = sim.info()
+            e0.record(stream)
+            while True:
+                sim.step(25)
+                sim.sync()
+                if sim.info().t - i0.t >= 1.0:
+                    break
+            e1.record(stream)
+            torch.cuda.synchronize()
+            i1 = sim.info()
+            row[tag] = {"seconds": e0.elapsed_time(e1) * 1e-3, "steps": int(i1.steps - i0.steps),
+                        "t_end": i1.t - i0.t,
+                        "sweeps_per_solve": (i1.iters_total - i0.iters_total) / max(i1.solves - i0.solves, 1)}
+            sim.close()
+            print(f"table2 n={n} {tag}: {row[tag]}", file=sys.stderr, flush=True)
+        rows.append(row)
+    print(json.dumps({"table2": rows, "unit": "seconds of the whole time loop to t >= 1",
+                      "note": "PAPER.md Table 2 workload; paper's numbers are on a GTX Titan Black"}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -336,7 +380,10 @@ def main():
     ap.add_argument("--solver", default="bicgstab", choices=["bicgstab", "srj"],
                     help="bicgstab: north_star solver (default); srj: the paper's scheduled-relaxation Jacobi")
     ap.add_argument("--srj-eps", type=float, default=1e-5, help="stopping tolerance of eq. (32) for --solver srj")
+    ap.add_argument("--table2", default="", help="comma-separated grid sizes: run the paper's Table 2 experiment instead")
     args = ap.parse_args()
+    if args.table2:
+        return run_table2(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_b200(args)

@@ -646,13 +646,15 @@ __global__ void __launch_bounds__(NT, 2) k_srj(SrjP P) {
   } else if (bmax == 0.0) {  // b = 0 => p~ = 0, zero iterations (same convention as solver 0)
     for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
       for (int I = threadIdx.x; I < G.nnx; I += NT) P.xA[nidx(G, I, J)] = 0.0;
-  } else if (!(rho < 1.0)) {
-    status = NH_ENOCONV;  // not strictly diagonally dominant: no bound on the spectrum
   } else {
-    // cycle length: smallest power of two with M sqrt(2 (1 - rho)) >= 7.6, at most mmax
-    const double gap = sqrt(2.0 * (1.0 - rho));
+    // cycle length: smallest power of two with M sqrt(2 (1 - rho)) >= 7.6, at most mmax.  Where a
+    // row is not strictly diagonally dominant (rho >= 1, e.g. across a discontinuous free surface)
+    // there is no interval to place Chebyshev nodes on: plain Jacobi (one factor, 1).
+    const bool dominant = rho < 1.0;
+    const double gap = dominant ? sqrt(2.0 * (1.0 - rho)) : 0.0;
     int M = 1;
-    while (M < P.mmax && (double)M * gap < 7.6) M *= 2;
+    if (dominant)
+      while (M < P.mmax && (double)M * gap < 7.6) M *= 2;
     const double* cosv = P.costab + (M - 1);
     const double tol = (P.rel > 0.0) ? P.rel * bmax : P.eps;
     // ghost images of the start vector
@@ -660,7 +662,7 @@ __global__ void __launch_bounds__(NT, 2) k_srj(SrjP P) {
       for (int I = threadIdx.x; I < G.nnx; I += NT) store_images(G, x, I, J, x[nidx(G, I, J)]);
     grid.sync();
     for (;;) {
-      const double om = 1.0 / (1.0 - rho * cosv[iters % M]);
+      const double om = dominant ? 1.0 / (1.0 - rho * cosv[iters % M]) : 1.0;
       unsigned long long* slot = &sc->srj_E_bits[iters % 3];
       srj_sweep(P, Q, om, x, xn, slot);
       grid.sync();

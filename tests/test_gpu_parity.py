@@ -509,3 +509,31 @@ def test_absorbing_zones_radial_hump_reduced(O, G):
                 dict(abs_xlo=1.0, gen_on=1, gen_A=0.1, gen_h0=0.5, gen_Lrel=1.0)):
         with pytest.raises(G.NHError):
             G.NH(16, 16, 0.1, 0.1, np.full((16, 16), 0.5), **bad)
+
+
+# ---------------------------------------------------------------- the paper's own timing workload
+def test_paper_dam_break_reduced_parity(O, G):
+    """Circular dam break of PAPER.md section 7.7 (Table 2) at 96 x 96: the paper's solver at its
+    loosest and tightest tolerance (bit-exact) and the default solver (within the tolerances)."""
+    cfg = inputs.paper_dam_break(96)
+    for eps in (1e-3, 1e-5):
+        o, g = both(O, G, cfg, solver=1, srj_eps=eps)
+        o.step(15)
+        g.step(15)
+        assert g.sync() == 0
+        so, sg = o.get_state(), g.get_state()
+        for k in so:
+            assert np.array_equal(so[k], sg[k]), (eps, k)
+        assert o.info().iters_total == g.info().iters_total and o.info().t == g.info().t
+    o, g = both(O, G, cfg)
+    o.step(15)
+    g.step(15)
+    assert g.sync() == 0
+    assert_parity(g.get_state(), o.get_state(), cfg["H"], cfg["h0"])
+    o, g = both(O, G, cfg, nonhydro=0)
+    o.step(15)
+    g.step(15)
+    assert g.sync() == 0
+    so, sg = o.get_state(), g.get_state()
+    for k in ("h", "qx", "qy"):
+        assert np.array_equal(so[k], sg[k]), k          # SWE path: bit-exact
