@@ -630,7 +630,10 @@ __device__ __forceinline__ void srj_sweep(const SrjP& P, const SolveP& Q, double
   }
 }
 
-__global__ void __launch_bounds__(NT, 2) k_srj(SrjP P) {
+#ifndef NH_SRJ_MINB
+#define NH_SRJ_MINB 2
+#endif
+__global__ void __launch_bounds__(NT, NH_SRJ_MINB) k_srj(SrjP P) {
   cg::grid_group grid = cg::this_grid();
   const NhGrid& G = P.G;
   NhScal* sc = P.sc;
