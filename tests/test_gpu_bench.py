@@ -1,0 +1,53 @@
+"""bench.py's JSON contract on a GPU box (-m gpu): one line, the driver's keys, the tier's roofline /
+cpu_baseline / e2e objects, for both solver modes and the reference arm."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+pytestmark = pytest.mark.gpu
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def _run(*args, env=None):
+    e = dict(os.environ, NH_BENCH_ORACLE_CROP="96")
+    e.update(env or {})
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), *args], capture_output=True, text=True,
+                       timeout=900, env=e)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1, r.stdout
+    return json.loads(lines[0])
+
+
+def test_bench_line_contract_small_config():
+    d = _run("--config", "3", "--nx", "256", "--ny", "192", "--steps", "3", "--warmup", "3")
+    for k in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "clocks", "e2e", "gpu_launches", "roofline", "cpu_baseline"):
+        assert k in d, k
+    assert d["unit"] == "cell-updates/s" and d["dtype"] == "f64" and d["data"] == "synthetic"
+    assert d["n_gpus"] == 1 and d["steps"] == 3 and d["warmup"] == 3 and d["higher_is_better"] is True
+    assert d["vs_baseline"] is None and "workload" in d["config"] and "model" not in d["config"]
+    assert d["value"] > 0 and abs(d["value"] - 256 * 192 * 3 / (d["ms_per_step"] * 3e-3)) <= 1e-6 * d["value"]
+    assert d["gpu_launches"] > 0 and d["config"]["status"] == [0, 0]
+    r = d["roofline"]
+    assert r["bound"] == "hbm" and r["unit"] == "GB/s" and r["peak"] > 1000 and r["achieved"] > 0
+    assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and "traffic" in r
+    e = d["e2e"]
+    assert e["value"] > 0 and e["h2d_bytes_per_step"] == e["d2h_bytes_per_step"] == 8 * (3 * 256 * 192 + 2 * 257 * 193)
+    assert e["value"] < d["value"] * 1.05           # host copies included: not faster than the device leg
+    c = d["cpu_baseline"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["sample"]
+    assert d["clocks"]["sm_mhz"] and d["clocks"]["sm_max_mhz"] and isinstance(d["clocks"]["reasons"], list)
+
+
+def test_bench_paper_solver_mode_and_reference_arm():
+    d = _run("--config", "3", "--nx", "256", "--ny", "192", "--steps", "3", "--warmup", "3", "--solver", "srj",
+             "--srj-eps", "1e-7", "--no-cpu")
+    assert "k_srj" in d["roofline"]["kernel"] and d["roofline"]["bytes_per_node_iteration"] == 56.0
+    assert "cpu_baseline" not in d and d["config"]["iters_per_solve"] > 1
+    ref = _run("--impl", "reference", "--steps", "1", "--warmup", "0")
+    assert ref["impl"] == "reference" and ref["value"] > 0 and ref["cpu_baseline"]["kind"] == "oracle"
+    assert ref["metric"] == d["metric"] and ref["unit"] == d["unit"]
