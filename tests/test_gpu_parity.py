@@ -537,3 +537,29 @@ def test_paper_dam_break_reduced_parity(O, G):
     so, sg = o.get_state(), g.get_state()
     for k in ("h", "qx", "qy"):
         assert np.array_equal(so[k], sg[k]), k          # SWE path: bit-exact
+
+
+# ---------------------------------------------------------------- strip / band boundaries of the solvers
+@pytest.mark.parametrize("nx", [57, 58, 59, 60, 61, 62, 119, 120, 121, 122])
+@pytest.mark.parametrize("bcs", [BCS[0], BCS[1]])
+def test_solvers_across_strip_boundaries(O, G, nx, bcs):
+    """The marching warps own 60-column strips with two halo lanes; grids whose last strip holds 1, 2
+    or 60 columns, periodic and mirror, both solvers: the solver-1 solve bit-exact, the BiCGStab solve
+    within the tolerance of two solves at 1e-12, and the true residual of both."""
+    ny = 13
+    cfg = rnd_cfg(nx, ny, bcs, seed=300 + nx, dry=0.1, dx=0.3, dy=0.3)
+    o, g = both(O, G, cfg)
+    b = o.rhs(0.02)
+    xo, ito, rro = o.solve(b)
+    xg, itg, rrg = g.solve(b)
+    assert rrg <= 1e-12 and abs(itg - ito) <= max(3, 0.15 * ito)
+    scale = np.max(np.abs(xo))
+    assert np.max(np.abs(xg - xo)) <= 1e-9 * scale
+    r = b - g.apply_A(xg)
+    nnx = nx if bcs[0] == PER else nx + 1
+    nny = ny if bcs[2] == PER else ny + 1
+    assert np.linalg.norm(r[:nny, :nnx]) <= 1.05e-12 * np.linalg.norm(b[:nny, :nnx])
+    o1, g1 = both(O, G, cfg, solver=1, srj_eps=1e-11)
+    xo1, ito1, Eo1 = o1.solve(b)
+    xg1, itg1, Eg1 = g1.solve(b)
+    assert ito1 == itg1 and Eo1 == Eg1 and np.array_equal(xo1, xg1)
