@@ -367,6 +367,38 @@ def run_table2(args):
     return 0
 
 
+def run_fullruns(args):
+    """Every listed BASELINE.json config at full size for its full number of steps (one nh_step call,
+    CUDA events around it): status, iterations, clamps, mass.  A robustness record, not the metric."""
+    import torch
+    from paper_1706_04551_b200 import inputs, nh
+    torch.cuda.set_device(0)
+    for idx in [int(x) for x in args.fullruns.split(",")]:
+        cfg = inputs.make_config(idx)
+        steps = cfg["steps"]
+        stream = torch.cuda.Stream()
+        g = nh.NH(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["H"], stream=stream, **cfg["params"])
+        g.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        g.step(steps)
+        e1.record(stream)
+        status = g.sync(allow=(nh.ENOCONV,))
+        torch.cuda.synchronize()
+        i, s = g.info(), g.get_state()
+        sec = e0.elapsed_time(e1) * 1e-3
+        m0 = float(np.sum(cfg["h"], dtype=np.longdouble))
+        m1 = float(np.sum(s["h"], dtype=np.longdouble))
+        print(json.dumps(dict(
+            config=idx, name=cfg["name"], nx=cfg["nx"], ny=cfg["ny"], steps=int(i.steps), seconds=sec,
+            cell_updates_per_s=cfg["nx"] * cfg["ny"] * steps / sec, status=int(status), t_end=i.t,
+            iters_per_solve=i.iters_total / max(i.solves, 1), iters_max=int(i.iters_max), res_last=i.res_last,
+            clamps=int(i.clamps), mass_rel_change=(m1 - m0) / m0,
+            finite=bool(all(np.isfinite(s[k]).all() for k in s)))), flush=True)
+        g.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -381,7 +413,10 @@ def main():
                     help="bicgstab: north_star solver (default); srj: the paper's scheduled-relaxation Jacobi")
     ap.add_argument("--srj-eps", type=float, default=1e-5, help="stopping tolerance of eq. (32) for --solver srj")
     ap.add_argument("--table2", default="", help="comma-separated grid sizes: run the paper's Table 2 experiment instead")
+    ap.add_argument("--fullruns", default="", help="comma-separated config numbers: run each at full size for its full step count")
     args = ap.parse_args()
+    if args.fullruns:
+        return run_fullruns(args)
     if args.table2:
         return run_table2(args)
     if args.impl == "reference":
