@@ -17,24 +17,29 @@ constexpr int BX = 32, BY = 8;
 
 struct Fld {  // read-only field + grid: ghost access S1 (R9)
   const NhGrid& G;
+  bool fast;  // every cell / node this thread touches is inside the grid: no index maps, no signs
   __device__ __forceinline__ double even(const double* __restrict__ a, int i, int j) const {
+    if (fast) return a[(size_t)j * G.nx + i];
     int ii = nh_map_cell_even(i, G.nx, G.bxlo, G.bxhi);
     int jj = nh_map_cell_even(j, G.ny, G.bylo, G.byhi);
     return a[(size_t)jj * G.nx + ii];
   }
   __device__ __forceinline__ double xn(const double* __restrict__ a, int i, int j) const {
+    if (fast) return a[(size_t)j * G.nx + i];
     double sx;
     int ii = nh_map_cell(i, G.nx, G.bxlo, G.bxhi, sx);
     int jj = nh_map_cell_even(j, G.ny, G.bylo, G.byhi);
     return sx * a[(size_t)jj * G.nx + ii];
   }
   __device__ __forceinline__ double yn(const double* __restrict__ a, int i, int j) const {
+    if (fast) return a[(size_t)j * G.nx + i];
     double sy;
     int ii = nh_map_cell_even(i, G.nx, G.bxlo, G.bxhi);
     int jj = nh_map_cell(j, G.ny, G.bylo, G.byhi, sy);
     return sy * a[(size_t)jj * G.nx + ii];
   }
   __device__ __forceinline__ double node(const double* __restrict__ a, int I, int J) const {
+    if (fast) return a[(size_t)J * G.np + I];
     int II = nh_map_node(I, G.nx, G.bxlo);
     int JJ = nh_map_node(J, G.ny, G.bylo);
     return a[(size_t)JJ * G.np + II];
@@ -49,6 +54,11 @@ struct Fld {  // read-only field + grid: ghost access S1 (R9)
     return 0.25 * (even(h, I - 1, J - 1) + even(h, I, J - 1) + even(h, I, J) + even(h, I - 1, J));
   }
 };
+
+// node (I,J) whose stencils (cells I-2..I+1, J-2..J+1; nodes I-1..I+1, J-1..J+1) stay inside the grid
+__device__ __forceinline__ bool node_interior(const NhGrid& G, int I, int J) {
+  return I >= 2 && I + 1 <= G.nx - 1 && J >= 2 && J + 1 <= G.ny - 1;
+}
 
 // z = 2 eta - h, eq. (6)
 __global__ void __launch_bounds__(256)
@@ -97,7 +107,7 @@ k_coeffs(NhGrid G, const double* __restrict__ h, const double* __restrict__ z,
          double* __restrict__ cW, double* __restrict__ cN, double* __restrict__ cS) {
   int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
   if (I >= G.nnx || J >= G.nny) return;
-  Fld F{G};
+  Fld F{G, node_interior(G, I, J)};
   double AC, AE, AW, AN, AS;
   node_coeffs(F, h, z, I, J, AC, AE, AW, AN, AS);
   size_t k = (size_t)J * G.np + I;
@@ -112,7 +122,7 @@ k_scale_coeffs(NhGrid G, const double* __restrict__ dinv, double* __restrict__ c
                double* __restrict__ cW, double* __restrict__ cN, double* __restrict__ cS) {
   int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
   if (I >= G.nnx || J >= G.nny) return;
-  Fld F{G};
+  Fld F{G, node_interior(G, I, J)};
   size_t k = (size_t)J * G.np + I;
   cE[k] = cE[k] * F.node(dinv, I + 1, J);
   cW[k] = cW[k] * F.node(dinv, I - 1, J);
@@ -161,7 +171,7 @@ k_apply_A(NhGrid G, const double* __restrict__ h, const double* __restrict__ z,
           const double* __restrict__ x, double* __restrict__ y) {
   int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
   if (I >= G.nnx || J >= G.nny) return;
-  Fld F{G};
+  Fld F{G, node_interior(G, I, J)};
   double AC, AE, AW, AN, AS;
   node_coeffs(F, h, z, I, J, AC, AE, AW, AN, AS);
   size_t k = (size_t)J * G.np + I;
@@ -195,7 +205,7 @@ k_rhs(NhGrid G, const NhScal* sc, int constraint_only, const double* __restrict_
       const double* __restrict__ w, double* __restrict__ b) {
   int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
   if (I >= G.nnx || J >= G.nny) return;
-  Fld F{G};
+  Fld F{G, node_interior(G, I, J)};
   size_t k = (size_t)J * G.np + I;
   double B = node_B(F, h, qx, qy, z, w[k], I, J);
   const double dt = sc->dt;
@@ -213,7 +223,7 @@ k_assemble_rows(NhGrid G, NhScal* sc, const double* __restrict__ h, const double
   int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
   double rad = 0.0, bm = 0.0;
   if (I < G.nnx && J < G.nny) {
-    Fld F{G};
+    Fld F{G, node_interior(G, I, J)};
     size_t k = (size_t)J * G.np + I;
     double AC, AE, AW, AN, AS;
     node_coeffs(F, h, z, I, J, AC, AE, AW, AN, AS);
@@ -343,7 +353,8 @@ k_correct_cells(NhGrid G, const NhScal* sc, const double* __restrict__ h,
                 double* __restrict__ qx_out, double* __restrict__ qy_out) {
   int i = blockIdx.x * BX + threadIdx.x, j = blockIdx.y * BY + threadIdx.y;
   if (i >= G.nx || j >= G.ny) return;
-  Fld F{G};
+  // cells i-1..i+1, j-1..j+1 and nodes i..i+1, j..j+1 inside the grid (periodic: node n wraps)
+  Fld F{G, i >= 1 && i <= G.nx - 2 && j >= 1 && j <= G.ny - 2};
   const double dt = sc->dt;
   size_t k = (size_t)j * G.nx + i;
   // corner nodes of cell (i,j): (i,j) (i+1,j) (i,j+1) (i+1,j+1)
@@ -364,7 +375,7 @@ k_correct_nodes(NhGrid G, const NhScal* sc, double delta, const double* __restri
                 double* __restrict__ w_out) {
   int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
   if (I >= G.nnx || J >= G.nny) return;
-  Fld F{G};
+  Fld F{G, node_interior(G, I, J)};
   size_t k = (size_t)J * G.np + I;
   double hn = F.hnode(h, I, J);
   w_out[k] = w2[k] + sc->dt * pt[k] * nh_dinv_h(hn, delta);
