@@ -83,9 +83,11 @@ typedef struct {
 typedef struct {
   double t;              /* simulated time                                                  */
   double dt_last;        /* last time step used                                             */
-  double res_last;       /* last solve: true ||b-Ax||_2/||b||_2 before the polish iteration */
+  double res_last;       /* last solve: solver 0: true ||b-Ax||_2/||b||_2 before the polish iteration;
+                            solver 1: the last max|Jacobi increment| E of eq. (32)           */
   long long steps;
-  long long iters_total; /* BiCGStab iterations over all solves (polish not counted)        */
+  long long iters_total; /* solver iterations over all solves (solver 0: BiCGStab iterations, polish
+                            not counted; solver 1: Jacobi sweeps that updated x)             */
   long long clamps;      /* number of h<0 -> 0 clamps in the predictor (R7)                 */
   long long solves;
   int iters_last, iters_max;
@@ -114,9 +116,11 @@ int nh_get_state(nh_ctx* ctx, double* h, double* qx, double* qy, double* w, doub
 
 /* nsteps full time steps: dt = CFL / max[(|u|+sqrt(gh))/dx + (|v|+sqrt(gh))/dy] (eq. (23),
  * DESIGN.md R20), then per Runge-Kutta stage: hydrostatic predictor (eqs (16)-(22), (30)),
- * breaking sources (eqs (8)-(12), (28)), pressure system assembly and BiCGStab solve (eqs
- * (24)-(29), (36)-(43)), Chorin-Temam correction (eqs (28), (31), (41)), relaxation zone
- * (L417-431); stages combined as U^{n+1} = (U^n + U^(2))/2 (L406, L516, L544). */
+ * semi-implicit Manning friction if manning_n > 0 (L61-65, L249), breaking sources (eqs (8)-(12),
+ * (28)), pressure system assembly and solve (eqs (24)-(29), (36)-(43); prm.solver: BiCGStab to
+ * solver_rtol, or the paper's Jacobi method with scheduled relaxation and rule (32)), Chorin-Temam
+ * correction (eqs (28), (31), (41)), generating / absorbing relaxation zones (L415-440); stages
+ * combined as U^{n+1} = (U^n + U^(2))/2 (L406, L516, L544). */
 int nh_step(nh_ctx* ctx, int nsteps);
 
 /* First part alone: predictor (S0-S5) on the current state, in place; w, p untouched.
@@ -141,7 +145,7 @@ long long nh_launch_count(nh_ctx* ctx);
  * synchronisation is added).  nh_profile_read synchronises, returns the summed milliseconds and
  * the number of brackets per phase since the last read (arrays of NH_PROF_CATS entries, HOST
  * pointers) and resets them.  Phases: the hydrostatic predictor (a1-a3), the assembly (a4-a5 and
- * the rows of A), the BiCGStab solve (a6: one cooperative kernel per bracket), and the correction
+ * the rows of A), the pressure solve (a6: one cooperative kernel per bracket), and the correction
  * with the Runge-Kutta combine (a7-a8). */
 enum { NH_PROF_PREDICTOR = 0, NH_PROF_ASSEMBLY = 1, NH_PROF_SOLVER = 2, NH_PROF_CORRECT = 3,
        NH_PROF_CATS = 4 };
@@ -154,8 +158,8 @@ int nh_apply_A(nh_ctx* ctx, const double* x_nodes, double* y_nodes); /* y = A(h,
 int nh_coeffs(nh_ctx* ctx, double* AC, double* AE, double* AW, double* AN, double* AS); /* rows of A */
 int nh_rhs(nh_ctx* ctx, double dt, double* b_nodes);      /* b = -B/dt of the current state (S7)   */
 int nh_constraint(nh_ctx* ctx, double* B_nodes);          /* discrete constraint B, eq. (37)       */
-/* S9 on the current state's operator: x_nodes in = start, out = solution; iters/relres are HOST
- * pointers (may be NULL); synchronises. */
+/* S9 on the current state's operator with the context's solver: x_nodes in = start, out = solution;
+ * iters/relres are HOST pointers (may be NULL; relres = res_last of nh_info); synchronises. */
 int nh_solve(nh_ctx* ctx, const double* b_nodes, double* x_nodes, int* iters, double* relres);
 
 #ifdef __cplusplus
