@@ -51,3 +51,23 @@ def test_bench_paper_solver_mode_and_reference_arm():
     ref = _run("--impl", "reference", "--steps", "1", "--warmup", "0")
     assert ref["impl"] == "reference" and ref["value"] > 0 and ref["cpu_baseline"]["kind"] == "oracle"
     assert ref["metric"] == d["metric"] and ref["unit"] == d["unit"]
+
+
+def test_bench_table2_and_fullruns_modes():
+    e = dict(os.environ)
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--table2", "64"], capture_output=True,
+                       text=True, timeout=600, env=e)
+    assert r.returncode == 0, r.stderr[-2000:]
+    d = json.loads([l for l in r.stdout.splitlines() if l.strip()][-1])
+    row = d["table2"][0]
+    assert row["n"] == 64 and all(k in row for k in ("swe", "nh_1e-3", "nh_1e-4", "nh_1e-5"))
+    assert all(row[k]["t_end"] >= 1.0 and row[k]["seconds"] > 0 for k in ("swe", "nh_1e-3", "nh_1e-4", "nh_1e-5"))
+    assert row["swe"]["sweeps_per_solve"] == 0.0
+    assert row["nh_1e-3"]["sweeps_per_solve"] <= row["nh_1e-4"]["sweeps_per_solve"] <= row["nh_1e-5"]["sweeps_per_solve"]
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--fullruns", "1,2"], capture_output=True,
+                       text=True, timeout=600, env=e)
+    assert r.returncode == 0, r.stderr[-2000:]
+    rows = [json.loads(l) for l in r.stdout.splitlines() if l.strip()]
+    assert [x["config"] for x in rows] == [1, 2] and all(x["status"] == 0 and x["finite"] for x in rows)
+    assert rows[0]["steps"] == 200 and rows[1]["steps"] == 1000 and rows[1]["iters_per_solve"] == 0.0
+    assert abs(rows[0]["mass_rel_change"]) < 1e-12 and rows[1]["mass_rel_change"] == 0.0
