@@ -48,6 +48,11 @@ namespace {
 constexpr int NT = 256, NW = NT / 32;  // CTA size, warps per CTA
 constexpr int SW = 60;                 // owned columns per warp strip
 constexpr int MAXDOT = 5;
+// small grids: at least this many rows per warp before CTAs are added (a warp marches its rows one
+// memory latency at a time; measured at 512 x 8 ... 512^2: 8 rows 18-20 us per iteration, 4 rows 13-15)
+#ifndef NH_MINROWS
+#define NH_MINROWS 4
+#endif
 
 struct SolveP {
   NhGrid G;
@@ -714,7 +719,7 @@ int nh_solver_setup(nh_ctx* c) {
   }
   const int nnx = c->g.nnx, nny = c->g.nny;
   const int nstrips = (nnx + SW - 1) / SW;
-  long long small_units = (long long)nstrips * ((nny + 7) / 8);
+  long long small_units = (long long)nstrips * ((nny + NH_MINROWS - 1) / NH_MINROWS);
   long long grid = (long long)occ * c->sm_count;
   if (grid > (small_units + NW - 1) / NW) grid = (small_units + NW - 1) / NW;
   if (grid < 1) grid = 1;
