@@ -563,3 +563,23 @@ def test_solvers_across_strip_boundaries(O, G, nx, bcs):
     xo1, ito1, Eo1 = o1.solve(b)
     xg1, itg1, Eg1 = g1.solve(b)
     assert ito1 == itg1 and Eo1 == Eg1 and np.array_equal(xo1, xg1)
+
+
+def test_everything_on_together(O, G):
+    """Breaking, friction, generating zone at x-lo, absorbing zones on the other open sides, wet/dry
+    bathymetry: solver 1 bit for bit, default solver within the tolerances."""
+    cfg = inputs.make_config(4, nx=384, ny=12)
+    extra = dict(manning_n=0.012, abs_xhi=0.0, bc_ylo=OUT, bc_yhi=OUT, abs_ylo=0.15, abs_yhi=0.2)
+    o, g = both(O, G, cfg, solver=1, srj_eps=1e-10, **extra)
+    o.step(40)
+    g.step(40)
+    assert g.sync() == 0
+    so, sg = o.get_state(), g.get_state()
+    assert np.array_equal(so["h"], sg["h"])
+    for k in ("qx", "qy", "w", "p"):      # cbrt in the friction factor: last-place differences allowed
+        assert np.max(np.abs(so[k] - sg[k])) <= 1e-12 * max(np.max(np.abs(so[k])), 1e-3), k
+    o, g = both(O, G, cfg, **extra)
+    o.step(40)
+    g.step(40)
+    assert g.sync() == 0
+    assert_parity(g.get_state(), o.get_state(), cfg["H"], cfg["h0"])
