@@ -583,3 +583,20 @@ def test_everything_on_together(O, G):
     g.step(40)
     assert g.sync() == 0
     assert_parity(g.get_state(), o.get_state(), cfg["H"], cfg["h0"])
+
+
+def test_bicgstab_is_bitwise_reproducible_from_run_to_run(G):
+    """Fixed-order two-stage dot products: the same problem gives the same bits every time."""
+    cfg = inputs.make_config(5, nx=320, ny=256)
+    outs = []
+    for _ in range(3):
+        g = G.NH(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["H"], **cfg["params"])
+        g.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
+        g.step(3)
+        assert g.sync() == 0
+        outs.append((g.get_state(), g.info().iters_total))
+        g.close()
+    for s, it in outs[1:]:
+        assert it == outs[0][1]
+        for k in s:
+            assert np.array_equal(s[k], outs[0][0][k]), k
