@@ -332,6 +332,13 @@ def run_table2(args):
     from paper_1706_04551_b200 import inputs, nh
     torch.cuda.set_device(0)
     sizes = [int(x) for x in args.table2.split(",")]
+    paper = {}   # the paper's printed seconds (tests/golden/table2_seconds.txt, cited there)
+    gp = os.path.join(ROOT, "tests", "golden", "table2_seconds.txt")
+    if os.path.exists(gp):
+        for line in open(gp):
+            f = line.split()
+            if f and not line.startswith("#"):
+                paper[int(f[0])] = dict(zip(("swe", "nh_1e-3", "nh_1e-4", "nh_1e-5"), map(float, f[1:5])))
     rows = []
     for n in sizes:
         cfg = inputs.paper_dam_break(n)
@@ -360,6 +367,9 @@ def run_table2(args):
                         "t_end": i1.t - i0.t,
                         "sweeps_per_solve": (i1.iters_total - i0.iters_total) / max(i1.solves - i0.solves, 1)}
             sim.close()
+            if n in paper:
+                row[tag]["paper_seconds_titan_black"] = paper[n][tag]
+                row[tag]["paper_over_b200"] = paper[n][tag] / row[tag]["seconds"]
             print(f"table2 n={n} {tag}: {row[tag]}", file=sys.stderr, flush=True)
         rows.append(row)
     print(json.dumps({"table2": rows, "unit": "seconds of the whole time loop to t >= 1",

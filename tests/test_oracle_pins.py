@@ -869,3 +869,13 @@ def test_srj_falls_back_to_plain_jacobi_where_dominance_is_lost(O):
     np.testing.assert_allclose(x.ravel(), y, rtol=0, atol=1e-12 * np.abs(y).max())
     # the increment rule underestimates the error by ~1/(1 - rho_Jacobi)
     np.testing.assert_allclose(x.ravel(), np.linalg.solve(A, b.ravel()), rtol=0, atol=1e-5 * np.abs(y).max())
+
+
+def test_golden_table2_fixture_is_well_formed():
+    # the paper's printed run times (Table 2): six grid sizes, four columns, increasing with
+    # the grid and with the tightness of epsilon
+    rows = [list(map(float, l.split())) for l in open(os.path.join(os.path.dirname(__file__), "golden",
+            "table2_seconds.txt")) if l.strip() and not l.startswith("#")]
+    assert [int(r[0]) for r in rows] == [250, 500, 750, 1000, 1250, 1500] and all(len(r) == 5 for r in rows)
+    a = np.array(rows)[:, 1:]
+    assert np.all(np.diff(a, axis=0) > 0) and np.all(np.diff(a, axis=1) >= 0)
