@@ -555,7 +555,6 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
  *     otherwise x <- x + omega z.  No dot products; every node update depends on x of the
  *     previous sweep only, so the result does not depend on the sweep order.
  * x: start -> solution.  res_out = the last E. */
-#define SRJ_PLAIN 32
 static int srj_solve(nho_ctx* c, const double* h, const double* z, const double* b, double* x,
                      int* iters_out, double* res_out) {
   const int nnx = c->nnx, nny = c->nny, maxit = c->prm.solver_maxit;
@@ -596,11 +595,13 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
   /* cycle length and schedule.  Where a row is not strictly diagonally dominant (rho >= 1: the
    * Gershgorin interval reaches 0; happens by a small margin along the bore of the paper's dam
    * break) the lower end of the spectrum is not bounded by the rows.  Reading R28: the solve then
-   * starts with SRJ_PLAIN plain Jacobi sweeps (factor 1: enough for the loose tolerances of (32)) and
-   * continues with Chebyshev cycles on [1 - rho_f, 1 + rho]: the upper end is the Gershgorin bound of
-   * the actual rows (rigorous; the polynomial explodes beyond it), the lower end that of the
-   * flat-bottom operator at the local depth (the smooth-flow value; an eigenvalue below it is still
-   * damped, only more slowly). */
+   * starts with plain Jacobi sweeps (factor 1: a few of them meet the loose tolerances of (32)) and
+   * looks at the decay of E every 4 sweeps (from sweep 8 on): with r4 = E_k / E_{k-4}, plain sweeps
+   * are predicted to reach E_k r4^(M/4) after another M; if that is still above the tolerance (or
+   * E does not decay) the solve switches, for good, to Chebyshev cycles on [1 - rho_f, 1 + rho]: the
+   * upper end is the Gershgorin bound of the actual rows (rigorous; the polynomial explodes beyond
+   * it), the lower end that of the flat-bottom operator at the local depth (the smooth-flow value;
+   * an eigenvalue below it is still damped, only more slowly). */
   const int dominant = (rho < 1.0);
   const double lo = dominant ? 1.0 - rho : 1.0 - rho_f, hi = 1.0 + rho;
   const double theta = 0.5 * (lo + hi), delta = 0.5 * (hi - lo);
@@ -620,13 +621,21 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
     double cosv = cos(3.14159265358979323846 * (double)(2 * perm[i] - 1) / (double)(2 * M));
     omega[i] = dominant ? 1.0 / (1.0 - rho * cosv) : 1.0 / (theta - delta * cosv);
   }
-  int iters = 0, status = NHO_OK;
-  double E = 0.0;
+  int iters = 0, status = NHO_OK, cyc_start = -1;
+  double E = 0.0, Esnap = 0.0;
   /* tolerance of (32): absolute (the paper's epsilon), or relative to max |b'| (R28) */
   const double tol = (c->prm.srj_rel > 0.0) ? c->prm.srj_rel * bmax : c->prm.srj_eps;
   for (;;) {
+    if (!dominant && cyc_start < 0 && iters >= 4 && iters % 4 == 0) {   /* E = E of sweep iters-1 */
+      if (iters >= 8) {
+        double r4 = E / Esnap, pw = r4;
+        for (int m = M / 4; m > 1; m >>= 1) pw = pw * pw;
+        if (!(r4 < 1.0) || E * pw > tol) cyc_start = iters;
+      }
+      Esnap = E;
+    }
     const double om = dominant ? omega[iters % M]
-                               : (iters < SRJ_PLAIN ? 1.0 : omega[(iters - SRJ_PLAIN) % M]);
+                               : (cyc_start < 0 ? 1.0 : omega[(iters - cyc_start) % M]);
     double Emax = 0.0;
     int nan = 0;
 #pragma omp parallel for if (c->ny >= 48) schedule(static) reduction(max : Emax) reduction(| : nan)
