@@ -561,9 +561,9 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
   double *dinv = c->kdiag, *ce = c->kph, *cw = c->ksh, *cn = c->ks, *cs = c->kt, *bp = c->kr;
   double *xn = c->kv;
   *iters_out = 0; *res_out = 0.0;
-  double rho = 0.0, rho_f = 0.0, bmax = 0.0;
+  double rho = 0.0, bmax = 0.0;
   int bad = 0;
-#pragma omp parallel for if (c->ny >= 48) schedule(static) reduction(max : rho, rho_f, bmax) reduction(| : bad)
+#pragma omp parallel for if (c->ny >= 48) schedule(static) reduction(max : rho, bmax) reduction(| : bad)
   for (int J = 0; J < nny; ++J)
     for (int I = 0; I < nnx; ++I) {
       double AC, AE, AW, AN, AS;
@@ -575,13 +575,6 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
       bp[k] = b[k] * di;
       double rad = ((fabs(ce[k]) + fabs(cw[k])) + fabs(cn[k])) + fabs(cs[k]);
       if (rad > rho) rho = rad;
-      {  /* Gershgorin radius of the FLAT-BOTTOM operator at the local depth (S8: A_C = 2 + kx + ky,
-          * off-diagonals -kx/2, -kx/2, -ky/2, -ky/2 with k = h_n^2 / Delta^2) */
-        double hn = node_geometry(c, h, z, I, J).hn;
-        double kx = hn * hn / (c->dx * c->dx), ky = hn * hn / (c->dy * c->dy);
-        double rf = (kx + ky) / (2.0 + kx + ky);
-        if (rf > rho_f) rho_f = rf;
-      }
       if (fabs(bp[k]) > bmax) bmax = fabs(bp[k]);
       if (!(bp[k] == bp[k]) || isinf(bp[k])) bad = 1;
     }
@@ -593,21 +586,13 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
     return NHO_OK;
   }
   /* cycle length and schedule.  Where a row is not strictly diagonally dominant (rho >= 1: the
-   * Gershgorin interval reaches 0; happens by a small margin along the bore of the paper's dam
-   * break) the lower end of the spectrum is not bounded by the rows.  Reading R28: the solve then
-   * starts with plain Jacobi sweeps (factor 1: a few of them meet the loose tolerances of (32)) and
-   * looks at the decay of E every 4 sweeps (from sweep 8 on): with r4 = E_k / E_{k-4}, plain sweeps
-   * are predicted to reach E_k r4^(M/4) after another M; if that is still above the tolerance (or
-   * E does not decay) the solve switches, for good, to Chebyshev cycles on [1 - rho_f, 1 + rho]: the
-   * upper end is the Gershgorin bound of the actual rows (rigorous; the polynomial explodes beyond
-   * it), the lower end that of the flat-bottom operator at the local depth (the smooth-flow value;
-   * an eigenvalue below it is still damped, only more slowly). */
+   * Gershgorin interval reaches 0, e.g. across a discontinuous free surface) there is no interval to
+   * place Chebyshev nodes on: the method falls back to the plain Jacobi method (one factor, 1). */
   const int dominant = (rho < 1.0);
-  const double lo = dominant ? 1.0 - rho : 1.0 - rho_f, hi = 1.0 + rho;
-  const double theta = 0.5 * (lo + hi), delta = 0.5 * (hi - lo);
-  const double gap = sqrt(2.0 * lo);
+  const double gap = dominant ? sqrt(2.0 * (1.0 - rho)) : 0.0;
   int M = 1;
-  while (M < c->prm.srj_mmax && (double)M * gap < 7.6) M *= 2;
+  if (dominant)
+    while (M < c->prm.srj_mmax && (double)M * gap < 7.6) M *= 2;
   int* perm = (int*)malloc(sizeof(int) * (size_t)M);
   double* omega = (double*)malloc(sizeof(double) * (size_t)M);
   if (!perm || !omega) { free(perm); free(omega); return NHO_ENOMEM; }
@@ -619,23 +604,14 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
     }
   for (int i = 0; i < M; ++i) {
     double cosv = cos(3.14159265358979323846 * (double)(2 * perm[i] - 1) / (double)(2 * M));
-    omega[i] = dominant ? 1.0 / (1.0 - rho * cosv) : 1.0 / (theta - delta * cosv);
+    omega[i] = dominant ? 1.0 / (1.0 - rho * cosv) : 1.0;
   }
-  int iters = 0, status = NHO_OK, cyc_start = -1;
-  double E = 0.0, Esnap = 0.0;
+  int iters = 0, status = NHO_OK;
+  double E = 0.0;
   /* tolerance of (32): absolute (the paper's epsilon), or relative to max |b'| (R28) */
   const double tol = (c->prm.srj_rel > 0.0) ? c->prm.srj_rel * bmax : c->prm.srj_eps;
   for (;;) {
-    if (!dominant && cyc_start < 0 && iters >= 4 && iters % 4 == 0) {   /* E = E of sweep iters-1 */
-      if (iters >= 8) {
-        double r4 = E / Esnap, pw = r4;
-        for (int m = M / 4; m > 1; m >>= 1) pw = pw * pw;
-        if (!(r4 < 1.0) || E * pw > tol) cyc_start = iters;
-      }
-      Esnap = E;
-    }
-    const double om = dominant ? omega[iters % M]
-                               : (cyc_start < 0 ? 1.0 : omega[(iters - cyc_start) % M]);
+    const double om = omega[iters % M];
     double Emax = 0.0;
     int nan = 0;
 #pragma omp parallel for if (c->ny >= 48) schedule(static) reduction(max : Emax) reduction(| : nan)
