@@ -19,11 +19,12 @@
  * (i+1/2,j+1/2) with i=I-1, j=J-1.  In a periodic direction the
  * last node line duplicates the first: ignored on input, filled on output.
  *
- * ASYNCHRONY.  nh_step / nh_hydrostatic_step / nh_nonhydro_correct / nh_set_state only enqueue
- * work on the context's stream and return (no host synchronisation inside; dt, the solver's
- * convergence tests and all reductions stay on the device).  nh_sync, nh_get_info, nh_get_state
- * to a pageable host buffer, and nh_last_error synchronise.  Sticky run-time conditions (a solve
- * that did not converge, a NaN time step) are reported by nh_sync / nh_get_info.
+ * ASYNCHRONY.  nh_step / nh_hydrostatic_step / nh_nonhydro_correct only enqueue work on the
+ * context's stream and return (no host synchronisation inside; dt, the solver's convergence tests
+ * and all reductions stay on the device).  nh_set_state, nh_get_state, nh_sync, nh_get_info and the
+ * test hooks synchronise with the stream (nh_set_state once, to report the validation of its
+ * input).  Sticky run-time conditions (a solve that did not converge, a NaN time step) are
+ * reported by nh_sync / nh_get_info.
  *
  * ERRORS.  0 on success, a negative nh_status otherwise; no exceptions, no aborts, no global
  * state.  One context may be used by one host thread at a time.
@@ -42,10 +43,10 @@ typedef enum { NH_BC_PERIODIC = 0, NH_BC_WALL = 1, NH_BC_OUTFLOW = 2 } nh_bc;
 
 typedef enum {
   NH_OK = 0,
-  NH_EINVAL = -1,  /* invalid argument (also: h < 0 or non-finite input found by nh_sync)  */
+  NH_EINVAL = -1,  /* invalid argument (also: h < 0 or non-finite input found by nh_set_state) */
   NH_ENOMEM = -2,  /* host or device allocation failed                                     */
   NH_ECUDA = -3,   /* a CUDA call failed (nh_last_error has the text)                      */
-  NH_ENOCONV = -4, /* a pressure solve hit maxit / broke down twice                        */
+  NH_ENOCONV = -4, /* a pressure solve hit maxit / still not converged after 8 restart cycles */
   NH_ENAN = -5     /* NaN/Inf time step or right-hand side                                 */
 } nh_status;
 
@@ -92,7 +93,7 @@ typedef struct {
   long long solves;
   int iters_last, iters_max;
   int flags;             /* bit0: a solve failed to converge; bit1: NaN/Inf dt or rhs;
-                            bit2: set_state saw h<0 or a non-finite value                   */
+                            bit2: the last set_state saw h<0 or a non-finite value (rejected) */
   int reserved;
 } nh_info;
 
@@ -108,8 +109,10 @@ int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* 
 void nh_destroy(nh_ctx* ctx);
 
 /* State = conserved variables (h, qx, qy) per cell (L45-59, L528) and (w, p) per staggered node
- * (L245-247, L464-466, L535).  w, p NULL => zeros.  set validates h >= 0 and finiteness on the
- * device (reported by nh_sync as NH_EINVAL, flag bit2). get: NULL => skip that field. */
+ * (L245-247, L464-466, L535).  w, p NULL => zeros.  set stages the arrays in a free slot,
+ * validates h >= 0 and finiteness there on the device, waits for that result (one stream
+ * synchronisation) and returns NH_EINVAL leaving the current state untouched if it fails.
+ * get: NULL => skip that field; synchronises (the arrays are complete on return). */
 int nh_set_state(nh_ctx* ctx, const double* h, const double* qx, const double* qy,
                  const double* w, const double* p);
 int nh_get_state(nh_ctx* ctx, double* h, double* qx, double* qy, double* w, double* p);
@@ -131,7 +134,7 @@ int nh_hydrostatic_step(nh_ctx* ctx, double dt);
 int nh_nonhydro_correct(nh_ctx* ctx, double dt);
 
 /* Wait for the stream; returns the sticky run-time status (NH_OK / NH_ENOCONV / NH_ENAN /
- * NH_EINVAL from set_state validation / NH_ECUDA) and clears nothing. */
+ * NH_ECUDA) and clears nothing. */
 int nh_sync(nh_ctx* ctx);
 int nh_get_info(nh_ctx* ctx, nh_info* out); /* synchronises */
 const char* nh_last_error(nh_ctx* ctx);

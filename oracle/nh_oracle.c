@@ -1121,6 +1121,18 @@ int nho_constraint(nho_ctx* c, double* B_nodes) {
   nodes_out(c, c->b, B_nodes);
   return NHO_OK;
 }
+int nho_breaking(nho_ctx* c, double dt, double* qx2, double* qy2, double* w2) {
+  if (!c || !qx2 || !qy2 || !w2 || !(dt > 0.0) || !c->prm.breaking) return NHO_EINVAL;
+  size_t nc = (size_t)c->nx * (size_t)c->ny;
+  memcpy(c->h1, c->h, nc * sizeof(double));
+  memcpy(c->qx1, c->qx, nc * sizeof(double));
+  memcpy(c->qy1, c->qy, nc * sizeof(double));
+  breaking_sources(c, c->w, dt);
+  memcpy(qx2, c->qx2, nc * sizeof(double));
+  memcpy(qy2, c->qy2, nc * sizeof(double));
+  nodes_out(c, c->w2, w2);
+  return NHO_OK;
+}
 int nho_solve(nho_ctx* c, const double* b_nodes, double* x_nodes, int* iters, double* relres) {
   if (!c || !b_nodes || !x_nodes) return NHO_EINVAL;
   int it = 0; double rr = 0.0;

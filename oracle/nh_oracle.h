@@ -88,6 +88,9 @@ int  nho_coeffs(nho_ctx* c, double* AC, double* AE, double* AW, double* AN, doub
 int  nho_rhs(nho_ctx* c, double dt, double* b_nodes);   /* b = -B/dt of the current state (S7), breaking ignored */
 int  nho_constraint(nho_ctx* c, double* B_nodes);       /* discrete B, eq. (37), current state */
 int  nho_solve(nho_ctx* c, const double* b_nodes, double* x_nodes, int* iters, double* relres); /* S9; x in: start */
+int  nho_breaking(nho_ctx* c, double dt, double* qx2, double* qy2, double* w2); /* S6 alone: the current
+                   state taken as U*, w -> q** = q* + dt R_u (cells), w** = w + dt R_w (nodes); updates the
+                   hysteresis flags of R11 (they persist across set_state); requires prm.breaking     */
 void nho_face_fluct(double g, double hm, double etam, double um, double vm,
                     double hp, double etap, double up, double vp,
                     double Dm[3], double Dp[3]);                     /* S4 */

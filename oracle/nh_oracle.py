@@ -63,6 +63,7 @@ def lib():
         L.nho_rhs.argtypes = [C.c_void_p, C.c_double, _dp]
         L.nho_constraint.argtypes = [C.c_void_p, _dp]
         L.nho_solve.argtypes = [C.c_void_p, _dp, _dp, C.POINTER(C.c_int), _dp]
+        L.nho_breaking.argtypes = [C.c_void_p, C.c_double, _dp, _dp, _dp]
         L.nho_face_fluct.argtypes = [C.c_double] * 9 + [_dp, _dp]
         L.nho_face_fluct.restype = None
         L.nho_dsg.argtypes = [C.c_double] * 3
@@ -179,6 +180,12 @@ class Oracle:
         b = np.empty(self.nshape)
         self._check(lib().nho_constraint(self._h, _ptr(b)))
         return b
+
+    def breaking(self, dt):
+        """S6 alone on the current state: -> dict(qx=q**_x, qy=q**_y, w=w**)."""
+        qx, qy, w = np.empty(self.cshape), np.empty(self.cshape), np.empty(self.nshape)
+        self._check(lib().nho_breaking(self._h, float(dt), _ptr(qx), _ptr(qy), _ptr(w)))
+        return dict(qx=qx, qy=qy, w=w)
 
     def solve(self, b, x0=None, allow_noconv=False):
         b = _c64(b, self.nshape)

@@ -28,7 +28,7 @@ def _nvcc():
 
 
 def _deps():
-    d = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f != "microbench_sweep.cu"]
+    d = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
     d.append(os.path.join(INC, "nh_b200.h"))
     d.append(os.path.abspath(__file__))
     return d
@@ -43,17 +43,6 @@ def build(force: bool = False, verbose: bool = False) -> str:
         ["-I", INC, "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.run(cmd, check=True, cwd=HERE)
     return LIB
-
-
-def build_microbench() -> str:
-    """Standalone microbenchmark of the solver's access pattern (csrc/microbench_sweep.cu)."""
-    out = os.path.join(HERE, "microbench_sweep")
-    src = os.path.join(CSRC, "microbench_sweep.cu")
-    if os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(src):
-        return out
-    subprocess.run([_nvcc(), "-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a",
-                    "--extended-lambda", "-o", out, src], check=True, cwd=HERE)
-    return out
 
 
 if __name__ == "__main__":

@@ -331,7 +331,14 @@ int nh_set_state(nh_ctx* c, const double* h, const double* qx, const double* qy,
     return fail(c, NH_EINVAL, "set_state: h<0 or non-finite input");
   c->cur = s1;
   if (node_in(c, c->w[c->curw], w) || node_in(c, c->p, p)) return NH_ECUDA;
+  // the CFL rate left by the last RK combine belongs to the replaced state: k_lambda takes a max
+  // onto lam_bits, so it has to start from zero (eq. (23) of the NEW state only)
   c->lam_valid = false;
+  if (cudaMemsetAsync(&c->sc->lam_bits, 0, sizeof(c->sc->lam_bits), c->stream) != cudaSuccess) {
+    (void)cudaGetLastError();
+    c->host_status = NH_ECUDA;
+    return fail(c, NH_ECUDA, "set_state: cudaMemsetAsync");
+  }
   return NH_OK;
 }
 
@@ -374,7 +381,7 @@ int nh_step(nh_ctx* c, int nsteps) {
       stage(c, s1, w1, s2, w2, 1);
       ProfScope ps(c, NH_PROF_CORRECT);
       nh_launch_combine(c, c->h[c->cur], c->qx[c->cur], c->qy[c->cur], c->w[c->curw], c->h[s2],
-                        c->qx[s2], c->qy[s2], c->w[w2]);
+                        c->qx[s2], c->qy[s2], w2 == c->curw ? nullptr : c->w[w2]);
       c->lam_valid = true;
     }
     nh_launch_end_step(c, 1);

@@ -298,8 +298,9 @@ k_combine(NhGrid G, double g, double delta, double* __restrict__ h0, double* __r
     double v = cfl_rate(g, delta, G.dx, G.dy, hv, qxv, qyv);
     if (v > l) l = v;
   }
-  for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < nn; k += stride)
-    w0[k] = 0.5 * w0[k] + 0.5 * w2[k];
+  if (w2 != nullptr)  // nullptr: w did not move in this step (hydrostatic path without zones)
+    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < nn; k += stride)
+      w0[k] = 0.5 * w0[k] + 0.5 * w2[k];
   block_max_to_global(l, &sc->lam_bits);
 }
 

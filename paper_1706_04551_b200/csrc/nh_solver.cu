@@ -7,7 +7,7 @@
 // host round trip per iteration (the paper's loop reads the error on the host every sweep,
 // L535-539).  Right preconditioning is folded into the operator: with M = diag(A) the iteration
 // runs on A M^-1 (unit diagonal, column-scaled off-diagonals cE..cS prepared once per solve by
-// k_scale_coeffs / k_ghost_coeffs) with the iterate y = M x; r is the residual of the
+// k_scale_coeffs) with the iterate y = M x; r is the residual of the
 // unpreconditioned system.
 //
 // Two passes over memory per iteration (d = one double per node):

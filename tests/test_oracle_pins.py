@@ -879,3 +879,244 @@ def test_golden_table2_fixture_is_well_formed():
     assert [int(r[0]) for r in rows] == [250, 500, 750, 1000, 1250, 1500] and all(len(r) == 5 for r in rows)
     a = np.array(rows)[:, 1:]
     assert np.all(np.diff(a, axis=0) > 0) and np.all(np.diff(a, axis=1) >= 0)
+
+
+# ---------------------------------------------------------------- generating relaxation zone
+# (U~ = m U + (1 - m) U*, w~, p~ with m_{i+-1/2} = (m_i + m_{i+-1}) / 2,
+# m_i = sqrt(1 - (d_i / L_Rel)^2); reading R18: d_i from the inner end of the zone, target = the
+# solitary wave (33) eta* = A sech^2(k (x - x0 - c t)), k = sqrt(3 A / (4 h0^3)),
+# c = sqrt(g (h0 + A)), q* = c eta*, w* = p* = 0, evaluated at the END time of the stage).
+def _solitary_target(x, t, g, A, h0, x0):
+    k = np.sqrt(3.0 * A / (4.0 * h0 ** 3))
+    c = np.sqrt(g * (h0 + A))
+    eta = A / np.cosh(k * (x - x0 - c * t)) ** 2
+    return eta, c * eta
+
+
+def _gen_zone_setup(O, time_order):
+    # a uniform current over a flat bottom is a fixed point of the finite-volume step (every flux
+    # difference vanishes, mirror ghosts at the open x boundary repeat it), so one first-order
+    # hydrostatic step leaves exactly the relaxation formula of L425-431
+    nx, ny, dx, dy, g, cfl = 48, 6, 0.25, 0.4, 9.81, 0.45
+    h0, a, qx0, qy0 = 0.8, 0.05, 0.3, -0.2
+    gen = dict(gen_on=1, gen_A=0.17, gen_h0=0.8, gen_x0=1.1, gen_Lrel=5.1)
+    H = np.full((ny, nx), h0)
+    st = inputs.random_smooth_state(nx, ny, dx, dy, seed=77)
+    o = O.Oracle(nx, ny, dx, dy, H, nonhydro=0, time_order=time_order, g=g, cfl=cfl,
+                 bc_xlo=OUT, bc_xhi=OUT, bc_ylo=PER, bc_yhi=PER, **gen)
+    U0 = dict(h=H + a, qx=np.full((ny, nx), qx0), qy=np.full((ny, nx), qy0), w=st["w"], p=st["p"])
+    t0 = 0.0
+    o.set_state(U0["h"], U0["qx"], U0["qy"], U0["w"], U0["p"])
+    hh = h0 + a
+    cc = np.sqrt(g * hh)
+    dt = cfl / ((abs(qx0 / hh) + cc) / dx + (abs(qy0 / hh) + cc) / dy)      # eq. (23), sum form (R20)
+    x = (np.arange(nx) + 0.5) * dx
+    L = gen["gen_Lrel"]
+    m = np.sqrt(1.0 - (np.clip(L - x, 0.0, L) / L) ** 2)                     # d from the inner end
+    mn = np.empty(nx + 1)
+    mn[1:nx] = 0.5 * (m[:-1] + m[1:])                                        # L429
+    mn[0], mn[nx] = 0.5 * m[0], 1.0              # no cell beyond the boundary (R18/R29); far side: no zone
+    return o, U0, dict(nx=nx, ny=ny, dx=dx, dy=dy, g=g, cfl=cfl, h0=h0, H=H, dt=dt, t0=t0, x=x, m=m,
+                       mn=mn, gen=gen)
+
+
+def test_generating_zone_closed_form_after_one_first_order_stage(O):
+    o, U0, P = _gen_zone_setup(O, time_order=1)
+    o.step(1)
+    s, info = o.get_state(), o.info()
+    assert info.dt_last == pytest.approx(P["dt"], rel=4e-16)
+    m, mn, gen = P["m"], P["mn"], P["gen"]
+    krel = int(np.ceil(gen["gen_Lrel"] / P["dx"]))
+    assert 0 < np.sum(m < 1.0) <= krel and m[0] < 0.4 and np.all(np.diff(m[:krel]) > 0)
+    eta_s, q_s = _solitary_target(P["x"], P["t0"] + P["dt"], P["g"], gen["gen_A"], gen["gen_h0"], gen["gen_x0"])
+    assert eta_s[:krel].max() > 0.2 * gen["gen_A"]          # the target is not negligible in the zone
+    for j in range(P["ny"]):
+        np.testing.assert_allclose(s["h"][j], m * U0["h"][j] + (1 - m) * (P["H"][j] + eta_s), rtol=0, atol=2e-15)
+        np.testing.assert_allclose(s["qx"][j], m * U0["qx"][j] + (1 - m) * q_s, rtol=0, atol=2e-15)
+        np.testing.assert_allclose(s["qy"][j], m * U0["qy"][j], rtol=0, atol=2e-15)
+    # node values: relaxed towards w* = p* = 0 with the mean of the two adjacent cell coefficients
+    nny = P["ny"]                                           # y periodic: distinct node lines 0..ny-1
+    np.testing.assert_allclose(s["w"][:nny], mn[None, :] * U0["w"][:nny], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(s["p"][:nny], mn[None, :] * U0["p"][:nny], rtol=0, atol=1e-15)
+    # outside the zone nothing moved
+    out = m == 1.0
+    assert np.array_equal(s["h"][:, out], U0["h"][:, out]) and np.array_equal(s["qx"][:, out], U0["qx"][:, out])
+
+
+def test_generating_zone_stage_clock_through_rk2(O):
+    # TVD-RK2 (L406, L544): U1 = relax(Phi(U^n), t + dt); U2 = relax(Phi(U1), t + 2 dt) -- the second
+    # stage starts from time t + dt, so its target is evaluated at t + 2 dt; U^{n+1} = (U^n + U2) / 2.
+    # Phi(U1) (U1 is no fixed point) is taken from a zone-free hydrostatic step of a second context.
+    o, U0, P = _gen_zone_setup(O, time_order=2)
+    o.step(1)
+    s = o.get_state()
+    m, gen, dt = P["m"], P["gen"], P["dt"]
+    e1, q1 = _solitary_target(P["x"], P["t0"] + dt, P["g"], gen["gen_A"], gen["gen_h0"], gen["gen_x0"])
+    e2, q2 = _solitary_target(P["x"], P["t0"] + 2 * dt, P["g"], gen["gen_A"], gen["gen_h0"], gen["gen_x0"])
+    U1 = dict(h=m * U0["h"] + (1 - m) * (P["H"] + e1[None, :]), qx=m * U0["qx"] + (1 - m) * q1[None, :],
+              qy=m * U0["qy"])
+    f = O.Oracle(P["nx"], P["ny"], P["dx"], P["dy"], P["H"], nonhydro=0, g=P["g"], cfl=P["cfl"],
+                 bc_xlo=OUT, bc_xhi=OUT, bc_ylo=PER, bc_yhi=PER)
+    f.set_state(U1["h"], U1["qx"], U1["qy"])
+    f.hydrostatic_step(dt)
+    F = f.get_state()
+    exp_h = 0.5 * U0["h"] + 0.5 * (m * F["h"] + (1 - m) * (P["H"] + e2[None, :]))
+    exp_qx = 0.5 * U0["qx"] + 0.5 * (m * F["qx"] + (1 - m) * q2[None, :])
+    exp_qy = 0.5 * U0["qy"] + 0.5 * (m * F["qy"])
+    np.testing.assert_allclose(s["h"], exp_h, rtol=0, atol=1e-14)
+    np.testing.assert_allclose(s["qx"], exp_qx, rtol=0, atol=1e-14)
+    np.testing.assert_allclose(s["qy"], exp_qy, rtol=0, atol=1e-14)
+    # the pin discriminates: the stage-1 clock in stage 2 would be off by far more than the tolerance
+    wrong = 0.5 * U0["h"] + 0.5 * (m * F["h"] + (1 - m) * (P["H"] + e1[None, :]))
+    assert np.max(np.abs(wrong - exp_h)) > 1e-4
+    # w, p: relaxed in both stages, w averaged with w^n; p is the second stage's (R19)
+    nny, mn = P["ny"], P["mn"]
+    np.testing.assert_allclose(s["w"][:nny], 0.5 * U0["w"][:nny] + 0.5 * (mn * mn)[None, :] * U0["w"][:nny],
+                               rtol=0, atol=1e-15)
+    np.testing.assert_allclose(s["p"][:nny], (mn * mn)[None, :] * U0["p"][:nny], rtol=0, atol=1e-15)
+    assert o.info().t == pytest.approx(dt, rel=4e-16)
+
+
+# ---------------------------------------------------------------- CFL time step, eq. (23)
+def test_cfl_time_step_closed_form(O):
+    # eq. (23) L339-341 per direction, summed over the two directions (R20):
+    # dt = CFL / max_ij [ (|u| + sqrt(g h)) / dx + (|v| + sqrt(g h)) / dy ]
+    nx, ny, dx, dy, g, cfl = 20, 12, 0.3, 0.7, 9.81, 0.6
+    H = np.full((ny, nx), 2.0)
+    for (h0, u, v) in [(2.0, 1.3, -0.4), (2.0, -2.1, 0.9), (0.5, 0.0, 3.0)]:
+        o = O.Oracle(nx, ny, dx, dy, H, g=g, cfl=cfl, bc_xlo=PER, bc_xhi=PER, bc_ylo=PER, bc_yhi=PER)
+        h = np.full((ny, nx), h0)
+        o.set_state(h, h * u, h * v)
+        c = np.sqrt(g * h0)
+        want = cfl / ((abs(u) + c) / dx + (abs(v) + c) / dy)
+        assert o.compute_dt() == pytest.approx(want, rel=4e-16)
+        # dropping a direction, a |.| or the celerity would be far off
+        assert abs(cfl / ((abs(u) + c) / dx) - want) > 0.05 * want
+        # one fast cell anywhere sets the maximum (here through v and the dy term alone)
+        qy = h * v
+        qy[7, 13] = h0 * (-9.0)
+        o.set_state(h, h * u, qy)
+        want1 = cfl / ((abs(u) + c) / dx + (9.0 + c) / dy)
+        assert o.compute_dt() == pytest.approx(want1, rel=4e-16) and want1 < want
+        # ... and one deep cell through sqrt(g h) in both terms
+        h2 = h.copy()
+        h2[3, 2] = 4.0 * h0
+        o.set_state(h2, h2 * u, h2 * v)
+        c2 = np.sqrt(g * 4.0 * h0)
+        assert o.compute_dt() == pytest.approx(cfl / ((abs(u) + c2) / dx + (abs(v) + c2) / dy), rel=4e-16)
+        # the step uses this dt and advances the clock by it (L406: t^{n+1} = t^n + dt)
+        o.set_state(h, h * u, h * v)
+        o.step(1)
+        assert o.info().dt_last == pytest.approx(want, rel=4e-16) and o.info().t == o.info().dt_last
+
+
+# ---------------------------------------------------------------- breaking sources: magnitudes
+def _breaking_1d_transcribed(h, q, H, w, dx, dt, g, B1, B2, flag_c, flag_n):
+    """Eqs (9)-(12), L136-165, L224 and the second stage of (28), L379-396, in 1D on interior cells
+    i = 1..n-2 and interior nodes (between cells i and i+1), transcribed from the paper:
+    nu = B h |q_x|, B = 1 - q_x / U1, U1,2 = B1,2 sqrt(g h); breaking starts when |q_x| >= U1 and goes
+    on while |q_x| >= U2; nu = 0 for B < 0; R_u = 2 nu u_x H_x, R_w = 2 nu u_x; cell derivatives
+    central (L394-396), node values by the compact formulas (25)."""
+    u = q / h
+    # cells
+    qx = (q[2:] - q[:-2]) / (2 * dx)
+    ux = (u[2:] - u[:-2]) / (2 * dx)
+    Hx = (H[2:] - H[:-2]) / (2 * dx)
+    hc = h[1:-1]
+    U1, U2 = B1 * np.sqrt(g * hc), B2 * np.sqrt(g * hc)
+    fc = (np.abs(qx) >= U1) | (flag_c & (np.abs(qx) >= U2))
+    nu = np.where(fc, np.maximum(1.0 - qx / U1, 0.0) * hc * np.abs(qx), 0.0)
+    q2 = q[1:-1] + dt * 2.0 * nu * ux * Hx
+    # nodes i+1/2, i = 0..n-2
+    hn = 0.5 * (h[1:] + h[:-1])
+    qxn = (q[1:] - q[:-1]) / dx
+    uxn = (u[1:] - u[:-1]) / dx
+    U1n, U2n = B1 * np.sqrt(g * hn), B2 * np.sqrt(g * hn)
+    fn = (np.abs(qxn) >= U1n) | (flag_n & (np.abs(qxn) >= U2n))
+    nun = np.where(fn, np.maximum(1.0 - qxn / U1n, 0.0) * hn * np.abs(qxn), 0.0)
+    w2 = w + dt * 2.0 * nun * uxn
+    return q2, w2, fc, fn, nu, nun
+
+
+def test_breaking_source_magnitudes_and_hysteresis_1d(O):
+    # y-invariant data: div q = q_x, div u = u_x, grad H = (H_x, 0): the 2D reading R12/R13 must
+    # reduce to the printed 1D formulas.  Linear q(x) on a plane beach H(x); B1 > B2 so that the
+    # "continues while |q_x| >= U2" branch (L143; R11) is a true hysteresis.
+    nx, ny, dx, dt, g, B1, B2 = 64, 5, 0.1, 0.013, 9.81, 0.4, 0.15
+    x = (np.arange(nx) + 0.5) * dx
+    Hrow = 1.6 - 0.2 * x                       # depth 1.59 .. 0.33: U1 = B1 sqrt(g h) from 1.58 down to 0.72
+    hrow = Hrow + 0.05 * np.cos(0.9 * x)
+    rng = np.random.Generator(np.random.PCG64(5))
+    wrow = rng.uniform(-0.3, 0.3, nx + 1)
+    H, h, w = np.tile(Hrow, (ny, 1)), np.tile(hrow, (ny, 1)), np.tile(wrow, (ny + 1, 1))
+    o = O.Oracle(nx, ny, dx, 0.37, H, g=g, breaking=1, B1=B1, B2=B2, bc_xlo=OUT, bc_xhi=OUT,
+                 bc_ylo=PER, bc_yhi=PER)
+    fresh = O.Oracle(nx, ny, dx, 0.37, H, g=g, breaking=1, B1=B1, B2=B2, bc_xlo=OUT, bc_xhi=OUT,
+                     bc_ylo=PER, bc_yhi=PER)
+    fc, fn = np.zeros(nx - 2, bool), np.zeros(nx - 1, bool)
+    seen = []
+    for k, gamma in enumerate((1.1, 0.62)):     # q_x = -gamma: 1st call flags the shallow part, 2nd keeps
+        qrow = 2.0 - gamma * x                  # it flagged where U2 <= |q_x| < U1 (hysteresis branch)
+        q = np.tile(qrow, (ny, 1))
+        o.set_state(h, q, 0 * h, w, None)
+        out = o.breaking(dt)
+        q2, w2, fc_new, fn_new, nu, nun = _breaking_1d_transcribed(hrow, qrow, Hrow, wrow[1:-1], dx, dt, g,
+                                                                   B1, B2, fc, fn)
+        for j in range(ny):
+            np.testing.assert_allclose(out["qx"][j, 1:-1], q2, rtol=1e-13, atol=0)
+            np.testing.assert_allclose(out["w"][j, 1:-1], w2, rtol=0, atol=1e-13 * np.abs(w2).max())
+        assert np.array_equal(out["qy"], 0 * h)                  # H_y = 0: no source in y
+        # the source is not small: a wrong factor 2, a missing B, h or |q_x| would show
+        assert np.max(np.abs(q2 - qrow[1:-1])) > 1e-4 and np.max(np.abs(w2 - wrow[1:-1])) > 1e-3
+        seen.append((fc_new.copy(), fn_new.copy(), nu.copy()))
+        if k == 1:
+            hyst = fc_new & ~(np.abs(-gamma) >= B1 * np.sqrt(g * hrow[1:-1]))
+            assert hyst.sum() >= 5                                # cells kept on only by the U2 rule
+            fresh.set_state(h, q, 0 * h, w, None)                 # no history: those cells do not break
+            outf = fresh.breaking(dt)
+            assert np.all(outf["qx"][2, 1:-1][hyst] == qrow[1:-1][hyst])
+            assert np.all(out["qx"][2, 1:-1][hyst] != qrow[1:-1][hyst])
+        fc, fn = fc_new, fn_new
+    assert 5 <= seen[0][0].sum() <= nx - 10                       # first call: flagged and unflagged cells
+    # rear-facing (q_x > 0) with |q_x| >= U1 everywhere: B = 1 - q_x/U1 <= 0 -> nu = 0 (L143-145)
+    qrow = 0.5 + 1.7 * x
+    o.set_state(h, np.tile(qrow, (ny, 1)), 0 * h, w, None)
+    out = o.breaking(dt)
+    assert np.array_equal(out["qx"], np.tile(qrow, (ny, 1))) and np.array_equal(out["w"], w)
+
+
+def test_breaking_sources_commute_with_transposition(O):
+    # the x <-> y mirror image of the previous data must give the mirrored sources (pins the y half
+    # of the 2D reading R12: div = d/dx + d/dy, grad H = (H_x, H_y))
+    st = inputs.random_smooth_state(40, 28, 0.1, 0.13, seed=12, depth=1.0)
+    prm = dict(breaking=1, B1=0.01, B2=0.004, bc_xlo=OUT, bc_xhi=WALL, bc_ylo=WALL, bc_yhi=OUT)
+    a = O.Oracle(40, 28, 0.1, 0.13, st["H"], **prm)
+    a.set_state(st["h"], st["qx"], st["qy"], st["w"], st["p"])
+    ra = a.breaking(0.01)
+    prmT = dict(breaking=1, B1=0.01, B2=0.004, bc_ylo=OUT, bc_yhi=WALL, bc_xlo=WALL, bc_xhi=OUT)
+    b = O.Oracle(28, 40, 0.13, 0.1, st["H"].T.copy(), **prmT)
+    b.set_state(st["h"].T.copy(), st["qy"].T.copy(), st["qx"].T.copy(), st["w"].T.copy(), st["p"].T.copy())
+    rb = b.breaking(0.01)
+    assert np.max(np.abs(ra["qx"] - st["qx"])) > 1e-6             # sources are active
+    np.testing.assert_allclose(rb["qy"].T, ra["qx"], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(rb["qx"].T, ra["qy"], rtol=0, atol=1e-15)
+    np.testing.assert_allclose(rb["w"].T, ra["w"], rtol=0, atol=1e-15)
+
+
+# ---------------------------------------------------------------- all-dry domain (reading R26)
+def test_all_dry_domain_is_left_unchanged(O):
+    # eq. (23) has no maximum over an empty wet set: dt = 0; b = -B/dt is read as 0, so p~ = 0 with
+    # zero iterations and the state (h, q, w) is unchanged
+    nx, ny = 24, 18
+    st = inputs.random_smooth_state(nx, ny, 1.0, 1.0, seed=3)
+    H = -1.0 - 0.3 * np.abs(st["H"])
+    z = np.zeros((ny, nx))
+    for order in (1, 2):
+        o = O.Oracle(nx, ny, 1.0, 1.0, H, time_order=order, breaking=1, bc_xlo=WALL, bc_xhi=OUT)
+        o.set_state(z, z, z, st["w"], st["p"])
+        assert o.compute_dt() == 0.0
+        assert o.step(3) == 0
+        s, i = o.get_state(), o.info()
+        assert i.dt_last == 0.0 and i.t == 0.0 and i.steps == 3 and i.iters_total == 0 and i.clamps == 0
+        assert all(np.all(s[k] == 0.0) for k in ("h", "qx", "qy", "p"))
+        assert np.array_equal(s["w"], st["w"])
