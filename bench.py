@@ -409,6 +409,85 @@ def run_fullruns(args):
     return 0
 
 
+def parity_ratios(go, oo, H, h0, g=9.81, tol=1e-9):
+    """error / allowed per field at the north_star bars (SURVEY 8(d) "Parity metric"): all <= 1 passes.
+    max|eta_g - eta_o| <= tol h0;  max|a_g - a_o| <= tol max(max|a_o|, 1e-3 floor_a) for a in qx, qy, w, p,
+    floors (h0 c0, h0 c0, c0, g h0), c0 = sqrt(g h0)."""
+    c0 = float(np.sqrt(g * h0))
+    out = {"eta": float(np.max(np.abs((go["h"] - H) - (oo["h"] - H))) / (tol * h0))}
+    for k, f in dict(qx=h0 * c0, qy=h0 * c0, w=c0, p=g * h0).items():
+        scale = max(float(np.max(np.abs(oo[k]))), 1e-3 * f)
+        out[k] = float(np.max(np.abs(go[k] - oo[k])) / (tol * scale))
+    return out
+
+
+def run_parityruns(args):
+    """Configured-horizon parity (north_star: "after the configured steps"): the CUDA path and the CPU
+    oracle advance the same seeded config side by side; at 10 checkpoints (every 10 % of the run) the
+    full states are compared at the north_star bars.  SPEC = idx:NXxNY:steps[:window], comma-separated.
+    One JSON line per run.  Slow (the oracle runs on the host cores): a record for profiles/, not the
+    driver's bench line."""
+    import torch
+    from oracle import nh_oracle
+    from paper_1706_04551_b200 import inputs, nh
+    torch.cuda.set_device(0)
+    for spec in args.parityruns.split(","):
+        f = spec.split(":")
+        idx, (nx, ny), steps = int(f[0]), map(int, f[1].lower().split("x")), int(f[2])
+        kw = dict(nx=nx, ny=ny)
+        if len(f) > 3:
+            kw["window"] = f[3]
+        cfg = inputs.make_config(idx, **kw)
+        prm = dict(cfg["params"])
+        o = nh_oracle.Oracle(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], **prm)
+        g = nh.NH(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], **prm)
+        for a in (o, g):
+            a.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
+        probe = nh_oracle.Oracle(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], **prm) if prm.get("breaking") else None
+        eps_dry = 1e-5
+        wet0 = int(np.sum(cfg["h"] > eps_dry))
+        cps, worst, done = [], 0.0, 0
+        t_o = t_g = 0.0
+        for k in range(10):
+            n = (steps * (k + 1)) // 10 - done
+            t0 = time.perf_counter(); o.step(n, allow_noconv=True); t_o += time.perf_counter() - t0
+            t0 = time.perf_counter(); g.step(n); stg = g.sync(allow=(nh.ENOCONV,)); t_g += time.perf_counter() - t0
+            done += n
+            so, sg = o.get_state(), g.get_state()
+            io, ig = o.info(), g.info()
+            r = parity_ratios(sg, so, cfg["H"], cfg["h0"])
+            worst = max(worst, max(r.values()))
+            wet = so["h"] > eps_dry
+            cp = dict(step=done, t_oracle=io.t, t_gpu=ig.t, ratios={a: round(b, 4) for a, b in r.items()},
+                      iters_total=[int(ig.iters_total), int(io.iters_total)], clamps=[int(ig.clamps), int(io.clamps)],
+                      wet_cells=int(wet.sum()), wet_cells_changed_vs_start=int(np.sum(wet != (cfg["h"] > eps_dry))),
+                      wet_mask_equal=bool(np.array_equal(wet, sg["h"] > eps_dry)),
+                      eta_max=float(np.max(np.where(wet, so["h"] - cfg["H"], -np.inf))), gpu_status=int(stg))
+            if probe is not None:   # where is the breaking criterion of (9) active right now? (oracle S6 hook)
+                probe.set_state(so["h"], so["qx"], so["qy"], so["w"], so["p"])
+                b = probe.breaking(max(io.dt_last, 1e-9))
+                cp["breaking_cells"] = int(np.sum((b["qx"] != so["qx"]) | (b["qy"] != so["qy"])))
+                cp["breaking_nodes"] = int(np.sum(b["w"] != so["w"]))
+            cps.append(cp)
+            print(f"parityrun {spec} step {done}/{steps}: worst ratio {max(r.values()):.3g} "
+                  f"(oracle {t_o:.0f} s, gpu {t_g:.1f} s)", file=sys.stderr, flush=True)
+        io, ig = o.info(), g.info()
+        print(json.dumps(dict(
+            parityrun=spec, workload=cfg["name"], nx=nx, ny=ny, dx=cfg["dx"], steps=steps, h0=cfg["h0"],
+            bars="max|d eta| <= 1e-9 h0; max|d a| <= 1e-9 max(max|a|, 1e-3 floor_a), a in qx,qy,w,p; ratio = error/allowed",
+            worst_ratio=worst, passed=bool(worst <= 1.0), checkpoints=cps, wet_cells_start=wet0,
+            clamp_hist_bins_m="<1e-15,<1e-12,<1e-9,<1e-6,<1e-3,>=1e-3",
+            clamp_hist_gpu=list(ig.clamp_hist), clamp_hist_oracle=list(io.clamp_hist),
+            clamp_max_gpu=ig.clamp_max, clamp_max_oracle=io.clamp_max,
+            mass_rel_change_oracle=float(np.sum(so["h"], dtype=np.longdouble) / np.sum(cfg["h"], dtype=np.longdouble) - 1),
+            oracle_seconds=t_o, gpu_seconds=t_g, oracle_threads=int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1)))),
+            flush=True)
+        g.close(); o.close()
+        if probe is not None:
+            probe.close()
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -424,7 +503,11 @@ def main():
     ap.add_argument("--srj-eps", type=float, default=1e-5, help="stopping tolerance of eq. (32) for --solver srj")
     ap.add_argument("--table2", default="", help="comma-separated grid sizes: run the paper's Table 2 experiment instead")
     ap.add_argument("--fullruns", default="", help="comma-separated config numbers: run each at full size for its full step count")
+    ap.add_argument("--parityruns", default="", help="idx:NXxNY:steps[:window],... : oracle beside the CUDA path over the "
+                    "configured horizon, parity at 10 checkpoints (slow; a record for profiles/)")
     args = ap.parse_args()
+    if args.parityruns:
+        return run_parityruns(args)
     if args.fullruns:
         return run_fullruns(args)
     if args.table2:

@@ -95,6 +95,9 @@ typedef struct {
   int flags;             /* bit0: a solve failed to converge; bit1: NaN/Inf dt or rhs;
                             bit2: the last set_state saw h<0 or a non-finite value (rejected) */
   int reserved;
+  double clamp_max;      /* largest |h*| of a clamped negative depth (R7, R24)             */
+  long long clamp_hist[6]; /* clamps by size of |h*| in metres: < 1e-15, < 1e-12, < 1e-9, < 1e-6,
+                            < 1e-3, >= 1e-3                                                 */
 } nh_info;
 
 void nh_default_params(nh_params* prm);
@@ -116,6 +119,10 @@ void nh_destroy(nh_ctx* ctx);
 int nh_set_state(nh_ctx* ctx, const double* h, const double* qx, const double* qy,
                  const double* w, const double* p);
 int nh_get_state(nh_ctx* ctx, double* h, double* qx, double* qy, double* w, double* p);
+/* Simulated time of the current state (default 0 at nh_create).  Together with nh_get_state /
+ * nh_set_state and nh_get_info().t this is the checkpoint / restart: the generating relaxation zone
+ * (L417-431) is the only part of the step that reads the clock.  Enqueued on the stream. */
+int nh_set_time(nh_ctx* ctx, double t);
 
 /* nsteps full time steps: dt = CFL / max[(|u|+sqrt(gh))/dx + (|v|+sqrt(gh))/dy] (eq. (23),
  * DESIGN.md R20), then per Runge-Kutta stage: hydrostatic predictor (eqs (16)-(22), (30)),
@@ -164,6 +171,11 @@ int nh_constraint(nh_ctx* ctx, double* B_nodes);          /* discrete constraint
 /* S9 on the current state's operator with the context's solver: x_nodes in = start, out = solution;
  * iters/relres are HOST pointers (may be NULL; relres = res_last of nh_info); synchronises. */
 int nh_solve(nh_ctx* ctx, const double* b_nodes, double* x_nodes, int* iters, double* relres);
+/* S6 alone (eqs (9)-(12), L136-165, L224; second stage of (28), L379-396): the current state taken
+ * as U*, -> q** = q* + dt R_u (cell arrays qx2, qy2) and w** = w + dt R_w (node array w2); updates
+ * the onset / termination flags of the breaking criterion (they persist across nh_set_state).
+ * Requires prm.breaking and dt > 0 (NH_EINVAL otherwise); synchronises. */
+int nh_breaking(nh_ctx* ctx, double dt, double* qx2, double* qy2, double* w2);
 
 #ifdef __cplusplus
 }

@@ -75,6 +75,10 @@ static int map_node(int I, int n, int bclo, int bchi) {
   return I;
 }
 
+/* OpenMP splits loops over rows when the grid is worth it (scheduling only: every reduction used is
+ * exact or has a fixed order, so results do not depend on the number of threads) */
+#define NHO_PAR(c) ((c)->ny >= 8 && (long long)(c)->nx * (c)->ny >= 4096)
+
 #define CIDX(c, i, j) ((size_t)(j) * (size_t)(c)->nx + (size_t)(i))
 #define NIDX(c, I, J) ((size_t)(J) * (size_t)((c)->nx + 1) + (size_t)(I))
 
@@ -128,7 +132,7 @@ double nho_minmod(double a, double b) {
 
 static void derived_fields(nho_ctx* c, const double* h, const double* qx, const double* qy) {
   const double delta = c->prm.delta;
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int j = 0; j < c->ny; ++j)
     for (int i = 0; i < c->nx; ++i) {
       size_t k = CIDX(c, i, j);
@@ -218,9 +222,10 @@ static void cell_slopes(const nho_ctx* c, const double* h, int i, int j, int dir
 /* in: (h,qx,qy) + derived fields; out: (h1,qx1,qy1).                                       */
 static void predictor(nho_ctx* c, const double* h, const double* qx, const double* qy, double dt) {
   const double g = c->prm.g;
-  long long clamps = 0;
+  long long clamps = 0, hist[6] = {0, 0, 0, 0, 0, 0};
+  double cmax = 0.0;
   derived_fields(c, h, qx, qy);
-#pragma omp parallel for if (c->ny >= 48) schedule(static) reduction(+ : clamps)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static) reduction(+ : clamps, hist[:6]) reduction(max : cmax)
   for (int j = 0; j < c->ny; ++j)
     for (int i = 0; i < c->nx; ++i) {
       double dU[2][3]; /* per direction: (h, normal q, tangential q) */
@@ -259,7 +264,13 @@ static void predictor(nho_ctx* c, const double* h, const double* qx, const doubl
       double hn = h[k] - lx * dU[0][0] - ly * dU[1][0];
       double qxn = qx[k] - lx * dU[0][1] - ly * dU[1][2];
       double qyn = qy[k] - lx * dU[0][2] - ly * dU[1][1];
-      if (hn < 0.0) { hn = 0.0; clamps++; }                 /* R7 */
+      if (hn < 0.0) {                                       /* R7; size statistics for R24 */
+        double a = -hn;
+        int bk = (a < 1e-15) ? 0 : (a < 1e-12) ? 1 : (a < 1e-9) ? 2 : (a < 1e-6) ? 3 : (a < 1e-3) ? 4 : 5;
+        hist[bk]++;
+        if (a > cmax) cmax = a;
+        hn = 0.0; clamps++;
+      }
       if (hn <= c->prm.eps_dry) { qxn = 0.0; qyn = 0.0; }   /* R7 */
       else if (c->prm.manning_n > 0.0) {
         /* Manning friction tau = g h u n^2 |u| / h^(4/3) (L61-65, L773-775), "discretized
@@ -274,13 +285,15 @@ static void predictor(nho_ctx* c, const double* h, const double* qx, const doubl
       c->h1[k] = hn; c->qx1[k] = qxn; c->qy1[k] = qyn;
     }
   c->info.clamps += clamps;
+  for (int k = 0; k < 6; ++k) c->info.clamp_hist[k] += hist[k];
+  if (cmax > c->info.clamp_max) c->info.clamp_max = cmax;
 }
 
 /* A4 / R20: dt = CFL / max_ij[(|u|+sqrt(gh))/dx + (|v|+sqrt(gh))/dy] */
 static double cfl_dt(nho_ctx* c, const double* h, const double* qx, const double* qy) {
   double lam = 0.0;
   const double g = c->prm.g, delta = c->prm.delta;
-#pragma omp parallel for if (c->ny >= 48) schedule(static) reduction(max : lam)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static) reduction(max : lam)
   for (int j = 0; j < c->ny; ++j)
     for (int i = 0; i < c->nx; ++i) {
       size_t k = CIDX(c, i, j);
@@ -344,7 +357,7 @@ static void node_coeffs(const nho_ctx* c, const double* h, const double* z, int 
 
 /* y = A x on the distinct nodes; neighbours through the node maps (R10). */
 static void apply_A(const nho_ctx* c, const double* h, const double* z, const double* x, double* y) {
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int J = 0; J < c->nny; ++J)
     for (int I = 0; I < c->nnx; ++I) {
       double AC, AE, AW, AN, AS;
@@ -374,7 +387,7 @@ static double node_B(const nho_ctx* c, const double* h, const double* qx, const 
 }
 
 static void compute_z(nho_ctx* c, const double* h, double* z) {
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int j = 0; j < c->ny; ++j)
     for (int i = 0; i < c->nx; ++i) {
       size_t k = CIDX(c, i, j);
@@ -386,7 +399,7 @@ static void compute_z(nho_ctx* c, const double* h, double* z) {
 /* dot products over the distinct nodes: row sums, then the sum of the row sums (fixed order) */
 static double dot_nodes(const nho_ctx* c, const double* a, const double* b2) {
   double* rows = (double*)malloc(sizeof(double) * (size_t)c->nny);
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int J = 0; J < c->nny; ++J) {
     double s = 0.0;
     for (int I = 0; I < c->nnx; ++I) s += a[NIDX(c, I, J)] * b2[NIDX(c, I, J)];
@@ -411,14 +424,14 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
   double bnorm = sqrt(dot_nodes(c, b, b));
   if (!(bnorm == bnorm) || isinf(bnorm)) return NHO_ENAN;
   if (bnorm == 0.0) {
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
     for (int J = 0; J < nny; ++J)
       for (int I = 0; I < nnx; ++I) x[NIDX(c, I, J)] = 0.0;
     return NHO_OK;
   }
   const double tol = rtol * bnorm;
   /* M = diag(A_C) */
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int J = 0; J < nny; ++J)
     for (int I = 0; I < nnx; ++I) {
       double AC, AE, AW, AN, AS;
@@ -430,7 +443,7 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
   for (int cycle = 0; cycle < 8 && !converged; ++cycle) {
     /* true residual r = b - A x */
     apply_A(c, h, z, x, r);
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
     for (int J = 0; J < nny; ++J)
       for (int I = 0; I < nnx; ++I) {
         size_t k = NIDX(c, I, J);
@@ -445,7 +458,7 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
       if (fabs(rho_new) < 1e-300) break;                    /* breakdown -> restart */
       double beta = (rho_new / rho) * (alpha / omega);
       rho = rho_new;
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
       for (int J = 0; J < nny; ++J)
         for (int I = 0; I < nnx; ++I) {
           size_t k = NIDX(c, I, J);
@@ -456,7 +469,7 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
       double sigma = dot_nodes(c, r0, v);
       if (fabs(sigma) < 1e-300) break;
       alpha = rho / sigma;
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
       for (int J = 0; J < nny; ++J)
         for (int I = 0; I < nnx; ++I) {
           size_t k = NIDX(c, I, J);
@@ -465,7 +478,7 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
       iters++;
       double snorm = sqrt(dot_nodes(c, s, s));
       if (snorm <= tol) {                                   /* half-step exit */
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
         for (int J = 0; J < nny; ++J)
           for (int I = 0; I < nnx; ++I) {
             size_t k = NIDX(c, I, J);
@@ -473,7 +486,7 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
           }
         break;
       }
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
       for (int J = 0; J < nny; ++J)
         for (int I = 0; I < nnx; ++I) {
           size_t k = NIDX(c, I, J);
@@ -484,7 +497,7 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
       if (tt == 0.0) break;
       omega = dot_nodes(c, t, s) / tt;
       if (fabs(omega) < 1e-300) break;
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
       for (int J = 0; J < nny; ++J)
         for (int I = 0; I < nnx; ++I) {
           size_t k = NIDX(c, I, J);
@@ -503,7 +516,7 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
   if (converged && rnorm > 0.0) {
     /* r, r0 hold the true residual; p = r */
     double rho = dot_nodes(c, r0, r);
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
     for (int J = 0; J < nny; ++J)
       for (int I = 0; I < nnx; ++I) {
         size_t k = NIDX(c, I, J);
@@ -513,7 +526,7 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
     double sigma = dot_nodes(c, r0, v);
     if (fabs(rho) >= 1e-300 && fabs(sigma) >= 1e-300) {
       double alpha = rho / sigma;
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
       for (int J = 0; J < nny; ++J)
         for (int I = 0; I < nnx; ++I) {
           size_t k = NIDX(c, I, J);
@@ -523,7 +536,7 @@ static int bicgstab(nho_ctx* c, const double* h, const double* z, const double* 
       apply_A(c, h, z, sh, t);
       double tt = dot_nodes(c, t, t);
       double omega = (tt > 0.0) ? dot_nodes(c, t, s) / tt : 0.0;
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
       for (int J = 0; J < nny; ++J)
         for (int I = 0; I < nnx; ++I) {
           size_t k = NIDX(c, I, J);
@@ -563,7 +576,7 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
   *iters_out = 0; *res_out = 0.0;
   double rho = 0.0, bmax = 0.0;
   int bad = 0;
-#pragma omp parallel for if (c->ny >= 48) schedule(static) reduction(max : rho, bmax) reduction(| : bad)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static) reduction(max : rho, bmax) reduction(| : bad)
   for (int J = 0; J < nny; ++J)
     for (int I = 0; I < nnx; ++I) {
       double AC, AE, AW, AN, AS;
@@ -580,7 +593,7 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
     }
   if (bad) return NHO_ENAN;
   if (bmax == 0.0) {  /* same convention as the BiCGStab path: b = 0 => p~ = 0, zero iterations */
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
     for (int J = 0; J < nny; ++J)
       for (int I = 0; I < nnx; ++I) x[NIDX(c, I, J)] = 0.0;
     return NHO_OK;
@@ -614,7 +627,7 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
     const double om = omega[iters % M];
     double Emax = 0.0;
     int nan = 0;
-#pragma omp parallel for if (c->ny >= 48) schedule(static) reduction(max : Emax) reduction(| : nan)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static) reduction(max : Emax) reduction(| : nan)
     for (int J = 0; J < nny; ++J)
       for (int I = 0; I < nnx; ++I) {
         size_t k = NIDX(c, I, J);
@@ -630,7 +643,7 @@ static int srj_solve(nho_ctx* c, const double* h, const double* z, const double*
     if (nan) { status = NHO_ENAN; break; }
     if (E < tol) break;                          /* eq. (32): x is the accepted iterate */
     if (iters >= maxit) { status = NHO_ENOCONV; break; }
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
     for (int J = 0; J < nny; ++J)
       for (int I = 0; I < nnx; ++I) x[NIDX(c, I, J)] = xn[NIDX(c, I, J)];
     iters++;
@@ -652,7 +665,7 @@ static void breaking_sources(nho_ctx* c, const double* w_in, double dt) {
   const double B1 = c->prm.B1, B2 = c->prm.B2;
   const double* h = c->h1;
   /* velocities of U* */
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int j = 0; j < c->ny; ++j)
     for (int i = 0; i < c->nx; ++i) {
       size_t k = CIDX(c, i, j);
@@ -660,7 +673,7 @@ static void breaking_sources(nho_ctx* c, const double* w_in, double dt) {
       c->v[k] = nho_dsg(h[k], c->qy1[k], delta);
     }
   /* cells: central differences (L394-396) */
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int j = 0; j < c->ny; ++j)
     for (int i = 0; i < c->nx; ++i) {
       size_t k = CIDX(c, i, j);
@@ -687,7 +700,7 @@ static void breaking_sources(nho_ctx* c, const double* w_in, double dt) {
       c->qy2[k] = c->qy1[k] + dt * (2.0 * nu * divu * Hy);
     }
   /* nodes: compact edge averages of (39) */
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int J = 0; J < c->nny; ++J)
     for (int I = 0; I < c->nnx; ++I) {
       size_t k = NIDX(c, I, J);
@@ -724,7 +737,7 @@ static void breaking_sources(nho_ctx* c, const double* w_in, double dt) {
 static void correction(nho_ctx* c, const double* pt, double dt, double* qx_out, double* qy_out,
                        double* w_out) {
   const double* h = c->h1; const double* z = c->z;
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int j = 0; j < c->ny; ++j)
     for (int i = 0; i < c->nx; ++i) {
       size_t k = CIDX(c, i, j);
@@ -737,7 +750,7 @@ static void correction(nho_ctx* c, const double* pt, double dt, double* qx_out, 
       qx_out[k] = c->qx2[k] - dt / (4.0 * c->dx) * ((2.0 * h[k] + xx) * pE + (xx - 2.0 * h[k]) * pW);
       qy_out[k] = c->qy2[k] - dt / (4.0 * c->dy) * ((2.0 * h[k] + xy) * pN + (xy - 2.0 * h[k]) * pS);
     }
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int J = 0; J < c->nny; ++J)
     for (int I = 0; I < c->nnx; ++I) {
       size_t k = NIDX(c, I, J);
@@ -762,7 +775,7 @@ static void relaxation(nho_ctx* c, double* h, double* qx, double* qy, double* w,
   const double cel = sqrt(c->prm.g * (h0 + A));
   int krel = (int)ceil(L / c->dx);
   if (krel > c->nx) krel = c->nx;
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int j = 0; j < c->ny; ++j)
     for (int i = 0; i < krel; ++i) {
       size_t k = CIDX(c, i, j);
@@ -775,7 +788,7 @@ static void relaxation(nho_ctx* c, double* h, double* qx, double* qy, double* w,
       qx[k] = m * qx[k] + (1.0 - m) * (cel * etas);
       qy[k] = m * qy[k];
     }
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int J = 0; J < c->nny; ++J)
     for (int I = 0; I <= krel && I < c->nnx; ++I) {
       size_t k = NIDX(c, I, J);
@@ -854,7 +867,7 @@ static int nonhydro_part(nho_ctx* c, const double* w_in, double dt, double* qx_o
   }
   compute_z(c, c->h1, c->z);
   /* S7: b = -B(U**, w**)/dt  (sign: R15) */
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
   for (int J = 0; J < c->nny; ++J)
     for (int I = 0; I < c->nnx; ++I)
       c->b[NIDX(c, I, J)] = (dt > 0.0) ? -node_B(c, c->h1, c->qx2, c->qy2, c->z, c->w2, I, J) / dt
@@ -1003,6 +1016,12 @@ int nho_get_state(nho_ctx* c, double* h, double* qx, double* qy, double* w, doub
   return NHO_OK;
 }
 
+int nho_set_time(nho_ctx* c, double t) {
+  if (!c || !(t == t) || isinf(t)) return NHO_EINVAL;
+  c->info.t = t;
+  return NHO_OK;
+}
+
 int nho_compute_dt(nho_ctx* c, double* dt) {
   if (!c || !dt) return NHO_EINVAL;
   *dt = cfl_dt(c, c->h, c->qx, c->qy);
@@ -1031,7 +1050,7 @@ int nho_step(nho_ctx* c, int nsteps) {
       st = stage(c, dt, c->info.t + dt);
       if (st == NHO_ENAN) return st;
       if (st != NHO_OK) worst = st;
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
       for (int j = 0; j < c->ny; ++j)
         for (int i = 0; i < c->nx; ++i) {
           size_t k = CIDX(c, i, j);
@@ -1039,7 +1058,7 @@ int nho_step(nho_ctx* c, int nsteps) {
           c->qx[k] = 0.5 * c->qx0[k] + 0.5 * c->qx[k];
           c->qy[k] = 0.5 * c->qy0[k] + 0.5 * c->qy[k];
         }
-#pragma omp parallel for if (c->ny >= 48) schedule(static)
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
       for (int J = 0; J < c->nny; ++J)
         for (int I = 0; I < c->nnx; ++I) {
           size_t k = NIDX(c, I, J);

@@ -64,6 +64,9 @@ typedef struct {
   int iters_last, iters_max;
   int flags;           /* bit0: a solve failed to converge                              */
   int reserved;
+  double clamp_max;    /* largest |h*| of a clamped negative depth (R7, R24)              */
+  long long clamp_hist[6]; /* clamps by size of |h*| in metres: < 1e-15, < 1e-12, < 1e-9, < 1e-6,
+                          < 1e-3, >= 1e-3                                                  */
 } nho_info;
 
 typedef struct nho_ctx nho_ctx;
@@ -75,6 +78,7 @@ void nho_destroy(nho_ctx* c);
 int  nho_set_state(nho_ctx* c, const double* h, const double* qx, const double* qy,
                    const double* w, const double* p);          /* w,p NULL => zeros     */
 int  nho_get_state(nho_ctx* c, double* h, double* qx, double* qy, double* w, double* p); /* NULL => skip */
+int  nho_set_time(nho_ctx* c, double t);          /* simulated time of the current state (restart) */
 int  nho_step(nho_ctx* c, int nsteps);            /* CFL dt each step, RK per time_order */
 int  nho_hydrostatic_step(nho_ctx* c, double dt); /* S0-S5 only, in place; dt<=0 => CFL  */
 int  nho_nonhydro_correct(nho_ctx* c, double dt); /* S6-S10 on the current state         */

@@ -32,6 +32,7 @@ class Info(C.Structure):
         ("steps", C.c_longlong), ("iters_total", C.c_longlong), ("clamps", C.c_longlong),
         ("solves", C.c_longlong),
         ("iters_last", C.c_int), ("iters_max", C.c_int), ("flags", C.c_int), ("reserved", C.c_int),
+        ("clamp_max", C.c_double), ("clamp_hist", C.c_longlong * 6),
     ]
 
 
@@ -51,6 +52,7 @@ def lib():
         L.nho_destroy.restype = None
         L.nho_set_state.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp]
         L.nho_get_state.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp]
+        L.nho_set_time.argtypes = [C.c_void_p, C.c_double]
         L.nho_step.argtypes = [C.c_void_p, C.c_int]
         L.nho_hydrostatic_step.argtypes = [C.c_void_p, C.c_double]
         L.nho_nonhydro_correct.argtypes = [C.c_void_p, C.c_double]
@@ -140,6 +142,9 @@ class Oracle:
         w, p = (np.empty(self.nshape) for _ in range(2))
         self._check(lib().nho_get_state(self._h, _ptr(h), _ptr(qx), _ptr(qy), _ptr(w), _ptr(p)))
         return dict(h=h, qx=qx, qy=qy, w=w, p=p)
+
+    def set_time(self, t):
+        self._check(lib().nho_set_time(self._h, float(t)))
 
     def step(self, nsteps=1, allow_noconv=False):
         return self._check(lib().nho_step(self._h, int(nsteps)), (ENOCONV,) if allow_noconv else ())

@@ -29,6 +29,7 @@ k_all_finite(size_t n, const double* __restrict__ a, int* bad) {
 }
 
 __global__ void k_clear_flag(NhScal* sc, int mask) { sc->flags &= ~mask; }
+__global__ void k_set_time(NhScal* sc, double t) { sc->t = t; }
 
 bool bc_ok(int b) { return b == NH_BC_PERIODIC || b == NH_BC_WALL || b == NH_BC_OUTFLOW; }
 
@@ -362,6 +363,13 @@ int nh_get_state(nh_ctx* c, double* h, double* qx, double* qy, double* w, double
   return NH_OK;
 }
 
+int nh_set_time(nh_ctx* c, double t) {
+  if (!c || !(t == t) || isinf(t)) return NH_EINVAL;
+  k_set_time<<<1, 1, 0, c->stream>>>(c->sc, t);
+  c->launches++;
+  return check_launch(c);
+}
+
 int nh_step(nh_ctx* c, int nsteps) {
   if (!c || nsteps < 0) return NH_EINVAL;
   if (c->host_status != NH_OK) return c->host_status;
@@ -434,6 +442,8 @@ int nh_get_info(nh_ctx* c, nh_info* out) {
   out->steps = s.steps; out->iters_total = s.iters_total; out->clamps = s.clamps;
   out->solves = s.solves; out->iters_last = s.iters_last; out->iters_max = s.iters_max;
   out->flags = s.flags;
+  memcpy(&out->clamp_max, &s.clamp_max_bits, sizeof(double));
+  for (int k = 0; k < 6; ++k) out->clamp_hist[k] = (long long)s.clamp_hist[k];
   return NH_OK;
 }
 
@@ -521,6 +531,19 @@ int nh_rhs(nh_ctx* c, double dt, double* b_nodes) {
 int nh_constraint(nh_ctx* c, double* B_nodes) {
   if (!c || !B_nodes) return NH_EINVAL;
   return rhs_hook(c, 1.0, B_nodes, 1);
+}
+
+int nh_breaking(nh_ctx* c, double dt, double* qx2, double* qy2, double* w2) {
+  if (!c || !qx2 || !qy2 || !w2 || !(dt > 0.0) || !c->prm.breaking) return NH_EINVAL;
+  nh_launch_set_dt(c, dt);
+  c->lam_valid = false;
+  nh_launch_breaking(c, c->h[c->cur], c->qx[c->cur], c->qy[c->cur], c->w[c->curw], c->qx2, c->qy2,
+                     c->w2);
+  size_t cb = c->nc * sizeof(double);
+  if (copy_async(c, qx2, c->qx2, cb) || copy_async(c, qy2, c->qy2, cb)) return NH_ECUDA;
+  if (node_out(c, c->w2, w2)) return NH_ECUDA;
+  cudaStreamSynchronize(c->stream);
+  return check_launch(c);
 }
 
 int nh_solve(nh_ctx* c, const double* b_nodes, double* x_nodes, int* iters, double* relres) {

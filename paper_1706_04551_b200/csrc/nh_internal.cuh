@@ -41,6 +41,9 @@ struct NhScal {
   unsigned long long srj_bmax_bits;  // max |b / A_C| (k_scale_rows)
   unsigned long long srj_E_bits[3];  // max |Jacobi increment| of sweep k in slot k % 3
   int srj_bad, pad2;                 // a NaN appeared in a sweep
+  // size statistics of the negative depths clamped by the predictor (R7, R24): exact integer atomics
+  unsigned long long clamp_max_bits;  // max |h*|, as the bits of a non-negative double
+  unsigned long long clamp_hist[6];   // < 1e-15, < 1e-12, < 1e-9, < 1e-6, < 1e-3, >= 1e-3 (metres)
 };
 
 enum { NH_FLAG_NOCONV = 1, NH_FLAG_NAN = 2, NH_FLAG_BADSTATE = 4 };

@@ -127,10 +127,9 @@ __device__ __forceinline__ void hi_face(const PredTile& T, int lx, int ly, int d
 #endif
 __global__ void __launch_bounds__(PTX* PTY, NH_PRED_MINB)
 k_predictor(NhGrid G, double g, double delta, double eps_dry, double manning_n, int order,
-            const NhScal* sc, const double* __restrict__ H, const double* __restrict__ h,
+            NhScal* sc, const double* __restrict__ H, const double* __restrict__ h,
             const double* __restrict__ qx, const double* __restrict__ qy,
-            double* __restrict__ h1, double* __restrict__ qx1, double* __restrict__ qy1,
-            unsigned long long* clamps) {
+            double* __restrict__ h1, double* __restrict__ qx1, double* __restrict__ qy1) {
   __shared__ PredTile T;
   __shared__ double DPx[3][PTY][PTX + 1];  // D^+ of the x-face on the low side of cell lx - PH
   __shared__ double DPy[3][PTY + 1][PTX];  // D^+ of the y-face on the low side of cell ly - PH
@@ -214,7 +213,14 @@ k_predictor(NhGrid G, double g, double delta, double eps_dry, double manning_n, 
   double hn = h[k] - lxr * dU[0][0] - lyr * dU[1][0];
   double qxn = qx[k] - lxr * dU[0][1] - lyr * dU[1][2];
   double qyn = qy[k] - lxr * dU[0][2] - lyr * dU[1][1];
-  if (hn < 0.0) { hn = 0.0; atomicAdd(clamps, 1ULL); }  // R7
+  if (hn < 0.0) {  // R7; size statistics for R24 (rare: integer atomics, exact and order independent)
+    double a = -hn;
+    int bk = (a < 1e-15) ? 0 : (a < 1e-12) ? 1 : (a < 1e-9) ? 2 : (a < 1e-6) ? 3 : (a < 1e-3) ? 4 : 5;
+    atomicAdd(&sc->clamp_hist[bk], 1ULL);
+    atomicMax(&sc->clamp_max_bits, (unsigned long long)__double_as_longlong(a));
+    atomicAdd((unsigned long long*)&sc->clamps, 1ULL);
+    hn = 0.0;
+  }
   if (hn <= eps_dry) { qxn = 0.0; qyn = 0.0; }          // R7
   else if (manning_n > 0.0) {
     // Manning friction tau = g h u n^2 |u| / h^(4/3) (L61-65, L773-775), semi-implicit (L249, R27):
@@ -343,7 +349,7 @@ void nh_launch_predictor(nh_ctx* c, const double* h, const double* qx, const dou
   dim3 grid((c->g.nx + PTX - 1) / PTX, (c->g.ny + PTY - 1) / PTY), block(PTX, PTY);
   k_predictor<<<grid, block, 0, c->stream>>>(c->g, c->prm.g, c->prm.delta, c->prm.eps_dry,
                                              c->prm.manning_n, c->prm.space_order, c->sc, c->H, h, qx, qy, h1, qx1,
-                                             qy1, (unsigned long long*)&c->sc->clamps);
+                                             qy1);
   c->launches++;
 }
 void nh_launch_combine(nh_ctx* c, double* h0, double* qx0, double* qy0, double* w0, const double* h2,

@@ -44,6 +44,7 @@ class Info(C.Structure):
         ("steps", C.c_longlong), ("iters_total", C.c_longlong), ("clamps", C.c_longlong),
         ("solves", C.c_longlong),
         ("iters_last", C.c_int), ("iters_max", C.c_int), ("flags", C.c_int), ("reserved", C.c_int),
+        ("clamp_max", C.c_double), ("clamp_hist", C.c_longlong * 6),
     ]
 
 
@@ -57,10 +58,10 @@ _lib = None
 _vp = C.c_void_p
 
 EXPORTS = (
-    "nh_default_params", "nh_create", "nh_destroy", "nh_set_state", "nh_get_state", "nh_step",
+    "nh_default_params", "nh_create", "nh_destroy", "nh_set_state", "nh_get_state", "nh_set_time", "nh_step",
     "nh_hydrostatic_step", "nh_nonhydro_correct", "nh_sync", "nh_get_info", "nh_last_error",
     "nh_launch_count", "nh_profile", "nh_profile_read", "nh_compute_dt", "nh_apply_A", "nh_coeffs",
-    "nh_rhs", "nh_constraint", "nh_solve",
+    "nh_rhs", "nh_constraint", "nh_solve", "nh_breaking",
 )
 
 
@@ -81,6 +82,7 @@ def lib():
         L.nh_destroy.restype = None
         L.nh_set_state.argtypes = [_vp] * 6
         L.nh_get_state.argtypes = [_vp] * 6
+        L.nh_set_time.argtypes = [_vp, C.c_double]
         L.nh_step.argtypes = [_vp, C.c_int]
         L.nh_hydrostatic_step.argtypes = [_vp, C.c_double]
         L.nh_nonhydro_correct.argtypes = [_vp, C.c_double]
@@ -98,6 +100,7 @@ def lib():
         L.nh_rhs.argtypes = [_vp, C.c_double, _vp]
         L.nh_constraint.argtypes = [_vp, _vp]
         L.nh_solve.argtypes = [_vp, _vp, _vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
+        L.nh_breaking.argtypes = [_vp, C.c_double, _vp, _vp, _vp]
         _lib = L
     return _lib
 
@@ -202,6 +205,9 @@ class NH:
         self._check(lib().nh_get_state(self._h, *ptrs))
         return out
 
+    def set_time(self, t):
+        self._check(lib().nh_set_time(self._h, float(t)))
+
     # ---- the path --------------------------------------------------------------------------
     def step(self, nsteps=1):
         self._check(lib().nh_step(self._h, int(nsteps)))
@@ -259,6 +265,11 @@ class NH:
         b = np.empty(self.nshape)
         self._check(lib().nh_constraint(self._h, b.ctypes.data))
         return b
+
+    def breaking(self, dt):
+        qx, qy, w = np.empty(self.cshape), np.empty(self.cshape), np.empty(self.nshape)
+        self._check(lib().nh_breaking(self._h, float(dt), qx.ctypes.data, qy.ctypes.data, w.ctypes.data))
+        return dict(qx=qx, qy=qy, w=w)
 
     def solve(self, b, x0=None, allow=()):
         keep = []

@@ -270,16 +270,73 @@ def test_minimum_grid_and_ragged_sizes(O, G):
 
 
 def test_all_dry_domain(O, G):
+    # reading R26 (eq. (23) has no maximum over an empty wet set): dt = 0, b = 0, p~ = 0, zero
+    # iterations, (h, q, w) unchanged -- compared with the oracle, whose behaviour is pinned on the
+    # CPU by test_all_dry_domain_is_left_unchanged
     nx, ny = 40, 24
-    H = -np.ones((ny, nx))
+    st = inputs.random_smooth_state(nx, ny, 1.0, 1.0, seed=3)
+    H = -1.0 - 0.3 * np.abs(st["H"])
     z = np.zeros((ny, nx))
-    g = G.NH(nx, ny, 1.0, 1.0, H)
-    g.set_state(z, z, z)
-    g.step(3)
-    assert g.sync() == 0
-    s = g.get_state()
-    assert all(np.all(s[k] == 0.0) for k in s)
-    assert g.info().dt_last == 0.0 and g.info().iters_total == 0
+    for order in (1, 2):
+        prm = dict(time_order=order, breaking=1, bc_xlo=WALL, bc_xhi=OUT)
+        g = G.NH(nx, ny, 1.0, 1.0, H, **prm)
+        o = O.Oracle(nx, ny, 1.0, 1.0, H, **prm)
+        for a in (g, o):
+            a.set_state(z, z, z, st["w"], st["p"])
+            a.step(3)
+        assert g.sync() == 0
+        sg, so = g.get_state(), o.get_state()
+        for k in so:
+            assert np.array_equal(sg[k], so[k]), k
+        assert np.array_equal(sg["w"], st["w"]) and np.all(sg["p"] == 0.0)
+        ig, io = g.info(), o.info()
+        assert ig.dt_last == io.dt_last == 0.0 and ig.t == io.t == 0.0
+        assert ig.iters_total == io.iters_total == 0 and ig.steps == io.steps == 3 and ig.clamps == io.clamps == 0
+
+
+def test_set_state_after_a_step_starts_the_cfl_rate_from_scratch(O, G):
+    # after a TVD-RK2 step the device holds the CFL rate of U^{n+1} (fused into the combine); a
+    # state set afterwards must get eq. (23) of ITS cells only, also when it is the slower one
+    fast = rnd_cfg(70, 37, BCS[1], seed=5, dry=0.1, dx=0.1, dy=0.1)
+    slow = inputs.random_smooth_state(70, 37, 0.1, 0.1, seed=6, depth=1.0, rough=0.05)
+    o, g = both(O, G, fast)
+    o.step(2)
+    g.step(2)
+    for a in (o, g):
+        a.set_state(slow["h"] * 0.04, slow["qx"] * 1e-3, slow["qy"] * 1e-3, slow["w"], slow["p"])
+    dto = o.compute_dt()
+    assert dto > 1.3 * o.info().dt_last                  # the new state allows a much longer step
+    assert g.compute_dt() == dto
+    o.step(1)
+    g.step(1)
+    assert g.sync() == 0 and g.info().dt_last == o.info().dt_last == dto
+    for a in (o, g):                                     # the same through nh_step directly
+        a.set_state(slow["h"] * 0.04, slow["qx"] * 1e-3, slow["qy"] * 1e-3, slow["w"], slow["p"])
+        a.step(1)
+    assert g.sync() == 0 and g.info().dt_last == o.info().dt_last == dto
+
+
+@pytest.mark.parametrize("bcs", BCS)
+def test_breaking_sources_bit_exact_with_hysteresis(O, G, bcs):
+    # S6 alone (eqs (9)-(12), L224), B1 > B2: the termination threshold keeps flagged cells and nodes
+    # breaking on the second call (R11); the oracle side is pinned by
+    # test_breaking_source_magnitudes_and_hysteresis_1d
+    cfg = rnd_cfg(70, 37, bcs, seed=13, dry=0.2, dx=0.1, dy=0.1, breaking=1, B1=0.05, B2=0.012)
+    o, g = both(O, G, cfg)
+    ro, rg = o.breaking(0.01), g.breaking(0.01)
+    for k in ro:
+        assert np.array_equal(ro[k], rg[k]), k
+    assert np.max(np.abs(ro["qx"] - cfg["qx"])) > 1e-8 and np.max(np.abs(ro["w"] - cfg["w"])) > 1e-6
+    for a in (o, g):                                     # weaker flow: only the hysteresis keeps nu > 0
+        a.set_state(cfg["h"], 0.5 * cfg["qx"], 0.5 * cfg["qy"], cfg["w"], cfg["p"])
+    ro2, rg2 = o.breaking(0.01), g.breaking(0.01)
+    for k in ro2:
+        assert np.array_equal(ro2[k], rg2[k]), k
+    o3, g3 = both(O, G, cfg)                             # without the history the result differs
+    o3.set_state(cfg["h"], 0.5 * cfg["qx"], 0.5 * cfg["qy"], cfg["w"], cfg["p"])
+    assert not np.array_equal(o3.breaking(0.01)["w"], ro2["w"])
+    with pytest.raises(G.NHError):
+        g.breaking(0.0)
 
 
 def test_invalid_arguments(G):
