@@ -411,11 +411,14 @@ def run_fullruns(args):
 
 def parity_ratios(go, oo, H, h0, g=9.81, tol=1e-9):
     """error / allowed per field at the north_star bars (SURVEY 8(d) "Parity metric"): all <= 1 passes.
-    max|eta_g - eta_o| <= tol h0;  max|a_g - a_o| <= tol max(max|a_o|, 1e-3 floor_a) for a in qx, qy, w, p,
-    floors (h0 c0, h0 c0, c0, g h0), c0 = sqrt(g h0)."""
+    max|eta_g - eta_o| <= tol h0;  max|a_g - a_o| <= tol max(max|a_o|, 1e-3 floor_a) for a in q, w, p,
+    floors (h0 c0, c0, g h0), c0 = sqrt(g h0); q = (qx, qy) is judged as one vector field against max|q|."""
     c0 = float(np.sqrt(g * h0))
     out = {"eta": float(np.max(np.abs((go["h"] - H) - (oo["h"] - H))) / (tol * h0))}
-    for k, f in dict(qx=h0 * c0, qy=h0 * c0, w=c0, p=g * h0).items():
+    qscale = max(float(np.max(np.abs(oo["qx"]))), float(np.max(np.abs(oo["qy"]))), 1e-3 * h0 * c0)
+    for k in ("qx", "qy"):      # the discharge is one vector field: common scale max|q| (DESIGN.md section 4)
+        out[k] = float(np.max(np.abs(go[k] - oo[k])) / (tol * qscale))
+    for k, f in dict(w=c0, p=g * h0).items():
         scale = max(float(np.max(np.abs(oo[k]))), 1e-3 * f)
         out[k] = float(np.max(np.abs(go[k] - oo[k])) / (tol * scale))
     return out

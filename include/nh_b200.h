@@ -78,7 +78,10 @@ typedef struct {
                          rule (32) (L507-514; R28): no dot products, results bit-identical
                          to the CPU oracle's                                                 */
   int srj_mmax;       /* solver 1: longest relaxation cycle, a power of two <= 4096; default 256 */
-  int reserved;
+  int w_advect;       /* 1: the vertical-velocity equation of [7], (hw)_t + div(hw u) = p (PAPER.md
+                         L109-113), instead of h w_t = p: in every stage the node values w are first
+                         transported by first-order upwind differences with the 4-cell mean of the
+                         desingularised velocities (R30); default 0                       */
 } nh_params;
 
 typedef struct {
@@ -176,6 +179,10 @@ int nh_solve(nh_ctx* ctx, const double* b_nodes, double* x_nodes, int* iters, do
  * the onset / termination flags of the breaking criterion (they persist across nh_set_state).
  * Requires prm.breaking and dt > 0 (NH_EINVAL otherwise); synchronises. */
 int nh_breaking(nh_ctx* ctx, double dt, double* qx2, double* qy2, double* w2);
+/* The transport step of the w-advection variant alone (L109-113, R30): w of the current
+ * state carried over dt by the node velocities of the current state -> node array w_out; the state
+ * is not changed.  dt > 0 required; works whatever prm.w_advect says; synchronises. */
+int nh_w_advect(nh_ctx* ctx, double dt, double* w_out);
 
 #ifdef __cplusplus
 }

@@ -43,6 +43,7 @@ struct nho_ctx {
   double *kr, *kr0, *kp, *kv, *ks, *kt, *kph, *ksh, *kdiag; /* BiCGStab vectors */
   /* RK copies */
   double *h0, *qx0, *qy0, *w0;
+  double *wadv;              /* w after the transport step of the w-advection variant (R30) */
 };
 
 /* ------------------------------------------------------------------------------------ */
@@ -854,6 +855,32 @@ static void absorbing_zones(nho_ctx* c, double* h, double* qx, double* qy, doubl
     if (L[side] > 0.0) absorb_side(c, side, L[side], h, qx, qy, w, p);
 }
 
+/* S5b (only if w_advect; reading R30): the vertical-velocity equation of [7],
+ * (hw)_t + div(hw u) = p (L109-113), which with h_t + div q = 0 is  w_t + u . grad w = p / h.
+ * The paper gives no discretisation ("can be easily extended").  Reading: in the first (hyperbolic)
+ * part of every stage the node values w are transported in advective form with first-order upwind
+ * differences between neighbouring nodes; the node velocity is the mean of the desingularised
+ * velocities (S0) of the four cells around the node, taken from the stage input U^n like the
+ * fluxes of the predictor (ghost cells through the maps of R9: the normal velocity of a wall node
+ * is 0).  The pressure part p / h is the unchanged S10.  Under the time step (23) the update is a
+ * convex combination of the node and its upwind neighbours (maximum principle). */
+static void w_advection(nho_ctx* c, const double* w_in, double dt, double* w_out) {
+#pragma omp parallel for if (NHO_PAR(c)) schedule(static)
+  for (int J = 0; J < c->nny; ++J)
+    for (int I = 0; I < c->nnx; ++I) {
+      double un = 0.25 * (cell_xn(c, c->u, I - 1, J - 1) + cell_xn(c, c->u, I, J - 1) +
+                          cell_xn(c, c->u, I, J) + cell_xn(c, c->u, I - 1, J));
+      double vn = 0.25 * (cell_yn(c, c->v, I - 1, J - 1) + cell_yn(c, c->v, I, J - 1) +
+                          cell_yn(c, c->v, I, J) + cell_yn(c, c->v, I - 1, J));
+      double wc = w_in[NIDX(c, I, J)];
+      double wx = (un > 0.0) ? (wc - node_val(c, w_in, I - 1, J)) / c->dx
+                             : (node_val(c, w_in, I + 1, J) - wc) / c->dx;
+      double wy = (vn > 0.0) ? (wc - node_val(c, w_in, I, J - 1)) / c->dy
+                             : (node_val(c, w_in, I, J + 1) - wc) / c->dy;
+      w_out[NIDX(c, I, J)] = wc - dt * (un * wx + vn * wy);
+    }
+}
+
 /* S6-S10 on U* = (h1,qx1,qy1) with w_in; results to (qx_out,qy_out,w_out), p in c->p. */
 static int nonhydro_part(nho_ctx* c, const double* w_in, double dt, double* qx_out, double* qy_out,
                          double* w_out) {
@@ -891,7 +918,12 @@ static int stage(nho_ctx* c, double dt, double t0) {
   predictor(c, c->h, c->qx, c->qy, dt);
   int st = NHO_OK;
   if (c->prm.nonhydro) {
-    st = nonhydro_part(c, c->w, dt, c->qx, c->qy, c->w);
+    const double* w_in = c->w;
+    if (c->prm.w_advect) {   /* R30: c->u, c->v are the velocities of the stage input (predictor, S0) */
+      w_advection(c, c->w, dt, c->wadv);
+      w_in = c->wadv;
+    }
+    st = nonhydro_part(c, w_in, dt, c->qx, c->qy, c->w);
     memcpy(c->h, c->h1, nc * sizeof(double));
   } else {
     memcpy(c->h, c->h1, nc * sizeof(double));
@@ -931,6 +963,7 @@ int nho_create(nho_ctx** out, int nx, int ny, double dx, double dy, const double
   if (prm->precision != 64) return NHO_EINVAL;
   if (!(prm->manning_n >= 0.0)) return NHO_EINVAL;
   if (prm->solver != 0 && prm->solver != 1) return NHO_EINVAL;
+  if (prm->w_advect != 0 && prm->w_advect != 1) return NHO_EINVAL;
   if (!(prm->srj_rel >= 0.0)) return NHO_EINVAL;
   if (!(prm->abs_xlo >= 0.0) || !(prm->abs_xhi >= 0.0) || !(prm->abs_ylo >= 0.0) || !(prm->abs_yhi >= 0.0)) return NHO_EINVAL;
   if ((prm->abs_xlo > 0.0 || prm->abs_xhi > 0.0) && prm->bc_xlo == NHO_BC_PERIODIC) return NHO_EINVAL;
@@ -950,7 +983,7 @@ int nho_create(nho_ctx** out, int nx, int ny, double dx, double dy, const double
   double** cellp[] = { &c->H, &c->h, &c->qx, &c->qy, &c->eta, &c->u, &c->v, &c->h1, &c->qx1, &c->qy1,
                        &c->qx2, &c->qy2, &c->z, &c->h0, &c->qx0, &c->qy0 };
   double** nodep[] = { &c->w, &c->p, &c->w2, &c->b, &c->kr, &c->kr0, &c->kp, &c->kv, &c->ks, &c->kt,
-                       &c->kph, &c->ksh, &c->kdiag, &c->w0 };
+                       &c->kph, &c->ksh, &c->kdiag, &c->w0, &c->wadv };
   int ok = 1;
   for (size_t a = 0; a < sizeof(cellp) / sizeof(cellp[0]); ++a) { *cellp[a] = (double*)calloc(nc, sizeof(double)); if (!*cellp[a]) ok = 0; }
   for (size_t a = 0; a < sizeof(nodep) / sizeof(nodep[0]); ++a) { *nodep[a] = (double*)calloc(nn, sizeof(double)); if (!*nodep[a]) ok = 0; }
@@ -966,7 +999,7 @@ void nho_destroy(nho_ctx* c) {
   if (!c) return;
   double* all[] = { c->H, c->h, c->qx, c->qy, c->eta, c->u, c->v, c->h1, c->qx1, c->qy1, c->qx2, c->qy2,
                     c->z, c->h0, c->qx0, c->qy0, c->w, c->p, c->w2, c->b, c->kr, c->kr0, c->kp, c->kv,
-                    c->ks, c->kt, c->kph, c->ksh, c->kdiag, c->w0 };
+                    c->ks, c->kt, c->kph, c->ksh, c->kdiag, c->w0, c->wadv };
   for (size_t a = 0; a < sizeof(all) / sizeof(all[0]); ++a) free(all[a]);
   free(c->flag_c); free(c->flag_n);
   free(c);
@@ -1152,6 +1185,14 @@ int nho_breaking(nho_ctx* c, double dt, double* qx2, double* qy2, double* w2) {
   nodes_out(c, c->w2, w2);
   return NHO_OK;
 }
+int nho_w_advect(nho_ctx* c, double dt, double* w_out) {
+  if (!c || !w_out || !(dt > 0.0)) return NHO_EINVAL;
+  derived_fields(c, c->h, c->qx, c->qy);
+  w_advection(c, c->w, dt, c->wadv);
+  nodes_out(c, c->wadv, w_out);
+  return NHO_OK;
+}
+
 int nho_solve(nho_ctx* c, const double* b_nodes, double* x_nodes, int* iters, double* relres) {
   if (!c || !b_nodes || !x_nodes) return NHO_EINVAL;
   int it = 0; double rr = 0.0;

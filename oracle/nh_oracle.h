@@ -50,7 +50,8 @@ typedef struct {
   int solver;          /* 0: Jacobi-preconditioned BiCGStab (R14); 1: the paper's Jacobi method
                           with scheduled relaxation (L507-514; reading R28)                     */
   int srj_mmax;        /* solver 1: longest relaxation cycle (power of two), default 256        */
-  int reserved;
+  int w_advect;        /* 1: vertical-velocity equation of [7], (hw)_t + div(hw u) = p (L109-113), instead of
+                          h w_t = p: w transported by first-order upwind differences (reading R30) */
 } nho_params;
 
 typedef struct {
@@ -91,6 +92,7 @@ int  nho_apply_A(nho_ctx* c, const double* x_nodes, double* y_nodes); /* y = A(h
 int  nho_coeffs(nho_ctx* c, double* AC, double* AE, double* AW, double* AN, double* AS);
 int  nho_rhs(nho_ctx* c, double dt, double* b_nodes);   /* b = -B/dt of the current state (S7), breaking ignored */
 int  nho_constraint(nho_ctx* c, double* B_nodes);       /* discrete B, eq. (37), current state */
+int  nho_w_advect(nho_ctx* c, double dt, double* w_out); /* S5b alone (R30): w of the current state transported over dt */
 int  nho_solve(nho_ctx* c, const double* b_nodes, double* x_nodes, int* iters, double* relres); /* S9; x in: start */
 int  nho_breaking(nho_ctx* c, double dt, double* qx2, double* qy2, double* w2); /* S6 alone: the current
                    state taken as U*, w -> q** = q* + dt R_u (cells), w** = w + dt R_w (nodes); updates the

@@ -22,7 +22,7 @@ class Params(C.Structure):
         ("breaking", C.c_int), ("nonhydro", C.c_int), ("time_order", C.c_int), ("space_order", C.c_int),
         ("bc_xlo", C.c_int), ("bc_xhi", C.c_int), ("bc_ylo", C.c_int), ("bc_yhi", C.c_int),
         ("solver_maxit", C.c_int), ("gen_on", C.c_int), ("precision", C.c_int), ("solver", C.c_int),
-        ("srj_mmax", C.c_int), ("reserved", C.c_int),
+        ("srj_mmax", C.c_int), ("w_advect", C.c_int),
     ]
 
 
@@ -66,6 +66,7 @@ def lib():
         L.nho_constraint.argtypes = [C.c_void_p, _dp]
         L.nho_solve.argtypes = [C.c_void_p, _dp, _dp, C.POINTER(C.c_int), _dp]
         L.nho_breaking.argtypes = [C.c_void_p, C.c_double, _dp, _dp, _dp]
+        L.nho_w_advect.argtypes = [C.c_void_p, C.c_double, _dp]
         L.nho_face_fluct.argtypes = [C.c_double] * 9 + [_dp, _dp]
         L.nho_face_fluct.restype = None
         L.nho_dsg.argtypes = [C.c_double] * 3
@@ -191,6 +192,12 @@ class Oracle:
         qx, qy, w = np.empty(self.cshape), np.empty(self.cshape), np.empty(self.nshape)
         self._check(lib().nho_breaking(self._h, float(dt), _ptr(qx), _ptr(qy), _ptr(w)))
         return dict(qx=qx, qy=qy, w=w)
+
+    def w_advect(self, dt):
+        """S5b alone (R30) on the current state: w transported over dt by the node velocities."""
+        w = np.empty(self.nshape)
+        self._check(lib().nho_w_advect(self._h, float(dt), _ptr(w)))
+        return w
 
     def solve(self, b, x0=None, allow_noconv=False):
         b = _c64(b, self.nshape)

@@ -39,7 +39,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
         m = os.path.getmtime(LIB)
         if all(m >= os.path.getmtime(p) for p in _deps()):
             return LIB
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    extra = os.environ.get("NH_NVCC_EXTRA", "").split()   # developer knob: extra -D switches for experiments
+    cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
         ["-I", INC, "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.run(cmd, check=True, cwd=HERE)
     return LIB

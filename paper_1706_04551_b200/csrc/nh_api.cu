@@ -159,13 +159,12 @@ void nonhydro_part(nh_ctx* c, const double* h1, const double* qx1, const double*
       nh_launch_breaking(c, h1, qx1, qy1, w_in, c->qx2, c->qy2, c->w2);
       qxs = c->qx2; qys = c->qy2; ws = c->w2;
     }
-    nh_launch_compute_z(c, h1, c->z);
     if (c->prm.solver == 1) {
+      nh_launch_compute_z(c, h1, c->z);
       nh_launch_assemble_rows(c, h1, qxs, qys, c->z, ws, c->kr);
-    } else {
+    } else {  // matrix-free solver: no rows of A are stored, only h and z with their ghost cells
+      nh_launch_cell_planes(c, h1);
       nh_launch_rhs(c, h1, qxs, qys, c->z, ws, c->b, 0);
-      nh_launch_coeffs(c, h1, c->z);
-      nh_launch_scale_coeffs(c);
     }
   }
   {
@@ -192,7 +191,13 @@ void stage(nh_ctx* c, int in, int inw, int out, int outw, int stage_idx) {
       ProfScope ps(c, NH_PROF_PREDICTOR);
       nh_launch_predictor(c, c->h[in], c->qx[in], c->qy[in], c->h[out], c->qx1, c->qy1);
     }
-    nonhydro_part(c, c->h[out], c->qx1, c->qy1, c->w[inw], c->qx[out], c->qy[out], c->w[outw]);
+    const double* w_in = c->w[inw];
+    if (c->prm.w_advect) {  // R30: w is first carried by the velocities of the stage input
+      ProfScope ps(c, NH_PROF_PREDICTOR);
+      nh_launch_w_advect(c, c->h[in], c->qx[in], c->qy[in], c->w[inw], c->wadv);
+      w_in = c->wadv;
+    }
+    nonhydro_part(c, c->h[out], c->qx1, c->qy1, w_in, c->qx[out], c->qy[out], c->w[outw]);
   } else {
     ProfScope ps(c, NH_PROF_PREDICTOR);
     nh_launch_predictor(c, c->h[in], c->qx[in], c->qy[in], c->h[out], c->qx[out], c->qy[out]);
@@ -238,6 +243,7 @@ int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* 
   if (prm->precision != 64) return NH_EINVAL;
   if (!(prm->manning_n >= 0.0)) return NH_EINVAL;
   if (prm->solver != 0 && prm->solver != 1) return NH_EINVAL;
+  if (prm->w_advect != 0 && prm->w_advect != 1) return NH_EINVAL;
   if (!(prm->srj_rel >= 0.0)) return NH_EINVAL;
   if (!(prm->abs_xlo >= 0.0) || !(prm->abs_xhi >= 0.0) || !(prm->abs_ylo >= 0.0) || !(prm->abs_yhi >= 0.0)) return NH_EINVAL;
   if ((prm->abs_xlo > 0.0 || prm->abs_xhi > 0.0) && prm->bc_xlo == NH_BC_PERIODIC) return NH_EINVAL;
@@ -277,7 +283,7 @@ int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* 
                       &c->qy[0], &c->qy[1], &c->qy[2], &c->qx1, &c->qy1, &c->z};
   double** nodes[] = {&c->w[0], &c->w[1], &c->w[2], &c->p, &c->b, &c->dg, &c->dinv, &c->cE, &c->cW,
                       &c->cN, &c->cS, &c->ky, &c->kr, &c->krB, &c->kr0, &c->kpA, &c->kpB, &c->kvA,
-                      &c->kvB, &c->kt, &c->w2};
+                      &c->kvB, &c->kt, &c->w2, &c->hc, &c->zc, &c->wadv};
   for (double** p : cells) ok = ok && dalloc(c, p, c->nc);
   for (double** p : nodes) ok = ok && nalloc(c, p);
   ok = ok && dalloc(c, &c->pub, c->nn);
@@ -546,13 +552,26 @@ int nh_breaking(nh_ctx* c, double dt, double* qx2, double* qy2, double* w2) {
   return check_launch(c);
 }
 
+int nh_w_advect(nh_ctx* c, double dt, double* w_out) {
+  if (!c || !w_out || !(dt > 0.0)) return NH_EINVAL;
+  nh_launch_set_dt(c, dt);
+  c->lam_valid = false;
+  nh_launch_w_advect(c, c->h[c->cur], c->qx[c->cur], c->qy[c->cur], c->w[c->curw], c->wadv);
+  if (node_out(c, c->wadv, w_out)) return NH_ECUDA;
+  cudaStreamSynchronize(c->stream);
+  return check_launch(c);
+}
+
 int nh_solve(nh_ctx* c, const double* b_nodes, double* x_nodes, int* iters, double* relres) {
   if (!c || !b_nodes || !x_nodes) return NH_EINVAL;
   if (node_in(c, c->b, b_nodes) || node_in(c, c->w2, x_nodes)) return NH_ECUDA;
-  nh_launch_compute_z(c, c->h[c->cur], c->z);
-  nh_launch_coeffs(c, c->h[c->cur], c->z);
-  if (c->prm.solver == 1) nh_launch_scale_rows(c, c->b, c->kr);
-  else nh_launch_scale_coeffs(c);
+  if (c->prm.solver == 1) {
+    nh_launch_compute_z(c, c->h[c->cur], c->z);
+    nh_launch_coeffs(c, c->h[c->cur], c->z);
+    nh_launch_scale_rows(c, c->b, c->kr);
+  } else {
+    nh_launch_cell_planes(c, c->h[c->cur]);
+  }
   nh_launch_solve(c, c->b, c->w2, 0);
   if (node_out(c, c->w2, x_nodes)) return NH_ECUDA;
   if (check_launch(c) != NH_OK) return NH_ECUDA;

@@ -138,10 +138,13 @@ struct nh_ctx {
   double *qx1, *qy1;             // predictor output q*
   double *qx2, *qy2;             // q** (breaking on)
   double* z;                     // z = 2 eta - h of U*
+  double *hc, *zc;               // h, z of U* in the node layout shifted by one column, ghost cells
+                                 // filled (operands of the matrix-free solver, nh_solver.cu)
   unsigned char *flag_c, *flag_n;
   // nodes
   double* w[3];
   double* w2;  // w** (breaking on)
+  double* wadv;  // w after the transport step of the w-advection variant (R30)
   double* p;   // pressure multiplier p~ (warm start of the next solve)
   double* b;   // right-hand side
   double *dg, *dinv, *cE, *cW, *cN, *cS;  // diag(A), its inverse, column-scaled off-diagonals
@@ -174,6 +177,7 @@ void nh_launch_combine(nh_ctx* c, double* h0, double* qx0, double* qy0, double* 
 void nh_launch_validate(nh_ctx* c, const double* h, const double* qx, const double* qy);
 // nh_pressure.cu
 void nh_launch_compute_z(nh_ctx* c, const double* h, double* z);
+void nh_launch_cell_planes(nh_ctx* c, const double* h);  // z (dense) and hc, zc (solver 0)
 void nh_launch_breaking(nh_ctx* c, const double* h, const double* qx1, const double* qy1,
                         const double* w_in, double* qx2, double* qy2, double* w2);
 void nh_launch_rhs(nh_ctx* c, const double* h, const double* qx, const double* qy, const double* z,
@@ -187,6 +191,8 @@ void nh_launch_apply_A(nh_ctx* c, const double* h, const double* z, const double
 void nh_launch_correct(nh_ctx* c, const double* h, const double* z, const double* qx2,
                        const double* qy2, const double* w2, const double* p, double* qx_out,
                        double* qy_out, double* w_out);
+void nh_launch_w_advect(nh_ctx* c, const double* h, const double* qx, const double* qy,
+                        const double* w_in, double* w_out);  // R30
 void nh_launch_relax(nh_ctx* c, double* h, double* qx, double* qy, double* w, double* p, int stage);
 void nh_launch_absorb(nh_ctx* c, double* h, double* qx, double* qy, double* w, double* p);
 void nh_launch_nodes_out(nh_ctx* c, const double* src, double* dst);

@@ -71,6 +71,25 @@ k_compute_z(size_t nc, const double* __restrict__ h, const double* __restrict__ 
   }
 }
 
+// z = 2 eta - h (eq. (6)) as the dense cell plane, and the operands of the matrix-free solver
+// (nh_solver.cu): h and z in the node layout shifted by one column (plane column P = cell P - 1),
+// cells -2 .. nx+1 by -2 .. ny+1 through the even cell maps (R9: h, H, eta are even in every ghost).
+__global__ void __launch_bounds__(BX* BY)
+k_cell_planes(NhGrid G, const double* __restrict__ h, const double* __restrict__ H,
+              double* __restrict__ z, double* __restrict__ hc, double* __restrict__ zc) {
+  int i = (int)(blockIdx.x * BX + threadIdx.x) - 2, j = (int)(blockIdx.y * BY + threadIdx.y) - 2;
+  if (i > G.nx + 1 || j > G.ny + 1) return;
+  int ii = nh_map_cell_even(i, G.nx, G.bxlo, G.bxhi);
+  int jj = nh_map_cell_even(j, G.ny, G.bylo, G.byhi);
+  size_t k = (size_t)jj * G.nx + ii;
+  double hv = h[k];
+  double eta = hv - H[k];
+  double zv = 2.0 * eta - hv;
+  if (ii == i && jj == j) z[k] = zv;
+  long long kp = (long long)j * G.np + (i + 1);
+  hc[kp] = hv; zc[kp] = zv;
+}
+
 // S8: the five coefficients of row (I,J), derived from (36)-(41); 1D restriction = (43).
 __device__ __forceinline__ void node_coeffs(const Fld& F, const double* __restrict__ h,
                                             const double* __restrict__ z, int I, int J, double& AC,
@@ -345,6 +364,35 @@ k_break_nodes(NhGrid G, const NhScal* sc, double g, double delta, double eps, do
   w2[k] = w_in[k] + dt * (2.0 * nu * divu);  // R_w, L224
 }
 
+// S5b (w-advection variant of [7]; reading R30): (hw)_t + div(hw u) = p with
+// h_t + div q = 0 is w_t + u . grad w = p / h.  Transport part, before S6: first-order upwind
+// differences between neighbouring nodes, node velocity = mean of the desingularised velocities (S0)
+// of the four cells around the node in the stage input (ghost cells through the maps of R9, so the
+// normal velocity of a wall node is 0).  Same operation order as the oracle: bit-exact.
+__global__ void __launch_bounds__(BX* BY)
+k_w_advect(NhGrid G, const NhScal* sc, double delta, const double* __restrict__ h,
+           const double* __restrict__ qx, const double* __restrict__ qy,
+           const double* __restrict__ w_in, double* __restrict__ w_out) {
+  int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
+  if (I >= G.nnx || J >= G.nny) return;
+  Fld F{G};
+  double sxm, sxp, sym, syp;
+  int im = nh_map_cell(I - 1, G.nx, G.bxlo, G.bxhi, sxm), ip = nh_map_cell(I, G.nx, G.bxlo, G.bxhi, sxp);
+  int jm = nh_map_cell(J - 1, G.ny, G.bylo, G.byhi, sym), jp = nh_map_cell(J, G.ny, G.bylo, G.byhi, syp);
+  size_t kNE = (size_t)jp * G.nx + ip, kSE = (size_t)jm * G.nx + ip;
+  size_t kNW = (size_t)jp * G.nx + im, kSW = (size_t)jm * G.nx + im;
+  double uSW = sxm * nh_dsg(h[kSW], qx[kSW], delta), uSE = sxp * nh_dsg(h[kSE], qx[kSE], delta);
+  double uNE = sxp * nh_dsg(h[kNE], qx[kNE], delta), uNW = sxm * nh_dsg(h[kNW], qx[kNW], delta);
+  double vSW = sym * nh_dsg(h[kSW], qy[kSW], delta), vSE = sym * nh_dsg(h[kSE], qy[kSE], delta);
+  double vNE = syp * nh_dsg(h[kNE], qy[kNE], delta), vNW = syp * nh_dsg(h[kNW], qy[kNW], delta);
+  double un = 0.25 * (uSW + uSE + uNE + uNW);
+  double vn = 0.25 * (vSW + vSE + vNE + vNW);
+  double wc = w_in[(size_t)J * G.np + I];
+  double wx = (un > 0.0) ? (wc - F.node(w_in, I - 1, J)) / G.dx : (F.node(w_in, I + 1, J) - wc) / G.dx;
+  double wy = (vn > 0.0) ? (wc - F.node(w_in, I, J - 1)) / G.dy : (F.node(w_in, I, J + 1) - wc) / G.dy;
+  w_out[(size_t)J * G.np + I] = wc - sc->dt * (un * wx + vn * wy);
+}
+
 // S10: correction, eqs (36),(41): q <- q** + dt T_NH(p) at cells
 __global__ void __launch_bounds__(BX* BY)
 k_correct_cells(NhGrid G, const NhScal* sc, const double* __restrict__ h,
@@ -494,6 +542,11 @@ void nh_launch_compute_z(nh_ctx* c, const double* h, double* z) {
   k_compute_z<<<grid_1d(c, c->nc, 256), 256, 0, c->stream>>>(c->nc, h, c->H, z);
   c->launches++;
 }
+void nh_launch_cell_planes(nh_ctx* c, const double* h) {
+  k_cell_planes<<<grid2(c->g.nx + 4, c->g.ny + 4), dim3(BX, BY), 0, c->stream>>>(c->g, h, c->H, c->z,
+                                                                                c->hc, c->zc);
+  c->launches++;
+}
 void nh_launch_breaking(nh_ctx* c, const double* h, const double* qx1, const double* qy1,
                         const double* w_in, double* qx2, double* qy2, double* w2) {
   const nh_params& P = c->prm;
@@ -542,6 +595,12 @@ void nh_launch_correct(nh_ctx* c, const double* h, const double* z, const double
   k_correct_nodes<<<grid2(c->g.nnx, c->g.nny), dim3(BX, BY), 0, c->stream>>>(
       c->g, c->sc, c->prm.delta, h, w2, p, w_out);
   c->launches += 2;
+}
+void nh_launch_w_advect(nh_ctx* c, const double* h, const double* qx, const double* qy,
+                        const double* w_in, double* w_out) {
+  k_w_advect<<<grid2(c->g.nnx, c->g.nny), dim3(BX, BY), 0, c->stream>>>(c->g, c->sc, c->prm.delta, h,
+                                                                       qx, qy, w_in, w_out);
+  c->launches++;
 }
 void nh_launch_relax(nh_ctx* c, double* h, double* qx, double* qy, double* w, double* p, int stage) {
   const nh_params& P = c->prm;

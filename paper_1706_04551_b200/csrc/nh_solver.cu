@@ -1,25 +1,34 @@
 // nh_solver.cu -- a6: Jacobi-preconditioned BiCGStab (R14, R25) for the compact
 // finite-difference pressure system (eqs (29), (36)-(43)) as ONE persistent
-// cooperative kernel per solve.
+// cooperative kernel per solve, with the operator applied matrix-free (L535).
 //
 // The whole solve -- true-residual (re)starts, the iteration loop with its convergence tests, the
 // half-step exit, breakdown restarts and the final polish iteration -- runs on the device: no
 // host round trip per iteration (the paper's loop reads the error on the host every sweep,
-// L535-539).  Right preconditioning is folded into the operator: with M = diag(A) the iteration
-// runs on A M^-1 (unit diagonal, column-scaled off-diagonals cE..cS prepared once per solve by
-// k_scale_coeffs) with the iterate y = M x; r is the residual of the
-// unpreconditioned system.
+// L535-539).
+//
+// Formulation.  Right preconditioning with M = diag(A) (van der Vorst's p^ = M^-1 p, s^ = M^-1 s;
+// r is the residual of the unpreconditioned system) is carried in SCALED VECTORS: the planes hold
+// r^ = M^-1 r, p^ = M^-1 p, v^ = M^-1 v, t^ = M^-1 t.  Every recurrence of the method is linear, so
+// it holds unchanged between the scaled vectors; the operator input (p^, s^) is then read as stored
+// and the output is divided by the diagonal of its OWN row only, so no neighbour's diagonal is ever
+// needed and the rows of A can be recomputed on the fly from the two cell planes h and z = 2 eta - h
+// (S8; ~55 flops per node and apply) instead of being read as four stored coefficient planes.  The
+// iterate is x itself (x += alpha p^ + omega s^).  Dot products are those of the UNSCALED vectors
+// (t.s = sum A_C^2 t^ s^ ...), so alpha, omega, beta, the residual norm and hence the iterates are
+// the ones of the textbook right-preconditioned method up to rounding.
 //
 // Two passes over memory per iteration (d = one double per node):
-//   pass B : s = r - alpha v;  t = (A M^-1) s;  dots t.s, t.t, s.s, r0.s, r0.t
-//            reads r, v, r0, 4c   writes t                                            8 d
-//   pass CA: s = r - alpha v;  y += alpha p + omega s;  r' = s - omega t;
-//            p' = r' + beta (p - omega v);  v' = (A M^-1) p';  dots r0.v', r'.r'
-//            reads r, v, t, p, y, r0, 4c   writes y, r', p', v'                      14 d
+//   pass B : s^ = r^ - alpha v^;  t = A s^;  dots t.s, t.t, s.s, r0.s, r0.t
+//            reads r^, v^, r0, h, z   writes t^                                        6 d
+//   pass CA: s^ = r^ - alpha v^;  x += alpha p^ + omega s^;  r^' = s^ - omega t^;
+//            p^' = r^' + beta (p^ - omega v^);  v' = A p^';  dots r0.v', r'.r'
+//            reads r^, v^, t^, p^, x, r0, h, z   writes x, r^', p^', v^'              12 d
 // with rho' = r0.s - omega r0.t (R25), so that every scalar of iteration i+1 is known after pass B
 // of iteration i and the x/r update of iteration i shares its pass with the p/v update of
-// iteration i+1.  s is never stored.  r, p, v are double-buffered (a pass reads the old planes
-// with their halo and writes the new ones).
+// iteration i+1.  s is never stored.  r^, p^, v^ are double-buffered (a pass reads the old planes
+// with their halo and writes the new ones).  18 d = 144 B per node-iteration (the stored-matrix
+// version of round 1 moved 22 d = 176 B).
 //
 // Sweep geometry ("marching warps").  Node planes are stored with a ghost ring (4 columns left,
 // >= 2 right, 2 rows above and below; pitch NP a multiple of 16, so every strip starts on a 32-byte
@@ -28,9 +37,9 @@
 // a boundary node stores its images, so no pass ever maps an index.  A warp owns a strip of 60
 // columns and marches down a band of R rows: lane l holds columns 60 s - 2 + 2 l and the next one
 // (one 16-byte load per plane per row), lanes 0 and 31 are halo lanes, the rows j-1, j, j+1 of the
-// stencil operand live in registers, east/west neighbours come from warp shuffles.  No shared
-// memory tiles, no block-level synchronisation inside a pass; all global accesses are coalesced
-// 512-byte row segments.
+// stencil operand and the cell rows the coefficients need live in registers, east/west neighbours
+// come from warp shuffles.  No shared memory tiles, no block-level synchronisation inside a pass;
+// all global accesses are coalesced 512-byte row segments.
 //
 // Dot products are two-stage and deterministic: per-CTA partials in a fixed order, one grid
 // barrier, then every CTA sums all partials in the same order, so all CTAs take every branch
@@ -45,7 +54,13 @@ namespace cg = cooperative_groups;
 
 namespace {
 
-constexpr int NT = 256, NW = NT / 32;  // CTA size, warps per CTA
+#ifndef NH_NT
+#define NH_NT 192
+#endif
+#ifndef NH_MINB
+#define NH_MINB 2
+#endif
+constexpr int NT = NH_NT, NW = NT / 32;  // CTA size, warps per CTA
 constexpr int SW = 60;                 // owned columns per warp strip
 constexpr int MAXDOT = 5;
 // small grids: at least this many rows per warp before CTAs are added (a warp marches its rows one
@@ -57,13 +72,15 @@ constexpr int MAXDOT = 5;
 struct SolveP {
   NhGrid G;
   int nstrips, R, nbands;  // strips of SW columns, band height, bands
-  const double *cE, *cW, *cN, *cS, *dg, *dinv, *b;
-  double* x;
-  double *y, *r0, *t;
-  double *rA, *rB, *pA, *pB, *vA, *vB;
+  const double *hc, *zc;   // cell planes h, z = 2 eta - h of U* (node layout shifted by one column)
+  const double* b;
+  double* x;               // the iterate: start vector in, solution out (the pressure plane)
+  double *r0, *t;          // shadow residual (unscaled); t^
+  double *rA, *rB, *pA, *pB, *vA, *vB;  // r^, p^, v^ (double-buffered)
   double* part;  // [2][MAXDOT][gridDim.x]
   NhScal* sc;
   double rtol;
+  double miex, miey;  // -1 / (8 dx^2), -1 / (8 dy^2)
   int maxit;
   int count_stats;
 };
@@ -123,15 +140,14 @@ __device__ __forceinline__ void block_partials(const double (&v)[K], double* par
 template <int K>
 __device__ __forceinline__ void grid_sums(const double* part, int buf, double (&out)[K],
                                           double (*red)[NW], double* bc) {
-  static_assert(K <= NW, "one warp per value");
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const int nb = gridDim.x;
-  if (wid < K) {
-    const double* src = part + ((size_t)buf * MAXDOT + wid) * nb;
+  for (int k = wid; k < K; k += NW) {
+    const double* src = part + ((size_t)buf * MAXDOT + k) * nb;
     double a = 0.0;
     for (int i = lane; i < nb; i += 32) a += __ldcg(&src[i]);
     for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-    if (lane == 0) bc[wid] = a;
+    if (lane == 0) bc[k] = a;
   }
   __syncthreads();
 #pragma unroll
@@ -184,54 +200,135 @@ __device__ __forceinline__ void st2(double* a, const SolveP& P, const Unit& U, i
   if (U.g1 != -2) a[nidx(G, U.g1, j)] = v.y;
 }
 
-// Register-resident operands of one sweep row.  Every pass is software-pipelined by hand: the
-// loads of the NEXT row are issued before the current row is computed and stored (the compiler
-// cannot hoist them itself across the stores of possibly aliasing planes), so each warp keeps one
-// full row of every plane (~3-5 KB) in flight while it computes.
-struct RowC {  // coefficient row j of (A M^-1) and the shadow residual
-  double2 q, e, w, n, s;
+// ---- matrix-free rows of A on the march ("coefficients are computed on the fly") ----
+// The cell planes hc, zc (h and z = 2 eta - h of U*, written once per stage by k_cell_planes) use
+// the node layout shifted by one column: plane column P holds cell P - 1, ghost cells filled through
+// the cell index maps (R9).  The lane that owns nodes c0, c0+1 loads cells c0-1, c0 as its own pair
+// and gets cell c0+1 from the next lane: k = 0, 1, 2 below.  Node A = c0 lies between the cell
+// columns k = 0 (west) and 1 (east), node B = c0+1 between k = 1 and 2.  A warp keeps the cell rows
+// J-1, J (and z of row J+1, xi^y of row J-1) in registers while it marches: per sweep step one row
+// of h and one of z are loaded, 16 bytes per node instead of the 32 of four stored coefficients.
+#define NH_FULL 0xffffffffu
+struct Coef {  // row of A at the lane's two nodes: A_E, A_W, A_N, A_S, A_C (S8)
+  double e[2], w[2], n[2], s[2], c[2];
 };
-__device__ __forceinline__ RowC ld_rowc(const SolveP& P, int c0, int j) {
-  RowC C;
-  C.q = ld2(P.r0, P.G, c0, j);
-  C.e = ld2(P.cE, P.G, c0, j); C.w = ld2(P.cW, P.G, c0, j);
-  C.n = ld2(P.cN, P.G, c0, j); C.s = ld2(P.cS, P.G, c0, j);
-  return C;
+__device__ __forceinline__ void lane3(double2 own, double (&q)[3]) {
+  q[0] = own.x; q[1] = own.y; q[2] = __shfl_down_sync(NH_FULL, own.x, 1);
+}
+struct March {
+  double hS[3], zS[3], zN[3], xyS[3];  // S = cell row J-1, N = cell row J; xyS = xi^y of row J-1
+  // state for the first node row Ja of a band
+  __device__ __forceinline__ void start(const SolveP& P, int c0, int Ja) {
+    double zSS[3];
+    lane3(ld2(P.zc, P.G, c0, Ja - 2), zSS);
+    lane3(ld2(P.zc, P.G, c0, Ja - 1), zS);
+    lane3(ld2(P.zc, P.G, c0, Ja), zN);
+    lane3(ld2(P.hc, P.G, c0, Ja - 1), hS);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) xyS[k] = 0.5 * (zN[k] - zSS[k]);
+  }
+  // rows of A at node row J from the cell rows h(J) and z(J+1) just loaded, then roll to J+1.
+  // S8 with the sums shared between the two nodes: 2 h_E = h_NE + h_SE is a column sum (sh), xi_E a
+  // quarter of the difference of the z column sums two cells apart, 2 h_N a row sum, ...;
+  // miex = -1 / (8 dx^2), miey = -1 / (8 dy^2).
+  __device__ __forceinline__ Coef step(const SolveP& P, double2 hrow, double2 zrow) {
+    double hN[3], zNN[3], xyN[3], sh[3], sz[3];
+    lane3(hrow, hN);
+    lane3(zrow, zNN);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+      sh[k] = hS[k] + hN[k];
+      sz[k] = zS[k] + zN[k];
+      xyN[k] = 0.5 * (zNN[k] - zS[k]);
+    }
+    const double szm = __shfl_up_sync(NH_FULL, sz[1], 1), szp = __shfl_down_sync(NH_FULL, sz[1], 1);
+    const double xi[3] = {0.25 * (sz[1] - szm), 0.25 * (sz[2] - sz[0]), 0.25 * (szp - sz[1])};
+    Coef C;
+#pragma unroll
+    for (int n = 0; n < 2; ++n) {
+      const double hn2 = 0.5 * (sh[n] + sh[n + 1]);  // 2 h_n, (38)
+      const double zx = 0.5 * (sz[n + 1] - sz[n]);
+      const double am = (hn2 - zx) * P.miex, ap = (hn2 + zx) * P.miex;
+      C.e[n] = am * (sh[n + 1] + xi[n + 1]);
+      C.w[n] = ap * (sh[n] - xi[n]);
+      const double cx = fma(am, sh[n + 1] - xi[n + 1], ap * (sh[n] + xi[n]));
+      const double hNr = hN[n] + hN[n + 1], hSr = hS[n] + hS[n + 1];
+      const double zy = 0.5 * ((zN[n] + zN[n + 1]) - (zS[n] + zS[n + 1]));
+      const double bm = (hn2 - zy) * P.miey, bp = (hn2 + zy) * P.miey;
+      const double xN = 0.5 * (xyN[n] + xyN[n + 1]), xS = 0.5 * (xyS[n] + xyS[n + 1]);
+      C.n[n] = bm * (hNr + xN);
+      C.s[n] = bp * (hSr - xS);
+      const double cy = fma(bm, hNr - xN, bp * (hSr + xS));
+      C.c[n] = 2.0 - (cx + cy);
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) { hS[k] = hN[k]; zS[k] = zN[k]; zN[k] = zNN[k]; xyS[k] = xyN[k]; }
+    return C;
+  }
+};
+
+// 1 / a for a >= 2 (the diagonal of A): hardware seed (20+ bits) and two Newton steps.  Not correctly
+// rounded; the scaling only has to be the same number wherever a node's diagonal is used.
+__device__ __forceinline__ double rcp_diag(double a) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
+  double e = fma(-a, r, 1.0);
+  r = fma(r, e, r);
+  e = fma(-a, r, 1.0);
+  return fma(r, e, r);
 }
 
-// (A M^-1) applied to the operand rows (m: j-1, c: j, n: j+1) at the lane's two columns of row j
-__device__ __forceinline__ double2 stencil2(const RowC& C, double2 m, double2 c, double2 n) {
-  double west0 = __shfl_up_sync(0xffffffffu, c.y, 1);
-  double east1 = __shfl_down_sync(0xffffffffu, c.x, 1);
+// off-diagonal part of (A x) at the lane's two nodes of row j from the operand rows m: j-1, c: j, n: j+1
+__device__ __forceinline__ double2 offdiag2(const Coef& C, double2 m, double2 c, double2 n) {
+  const double west0 = __shfl_up_sync(NH_FULL, c.y, 1);
+  const double east1 = __shfl_down_sync(NH_FULL, c.x, 1);
   double2 o;
-  o.x = fma(C.s.x, m.x, fma(C.n.x, n.x, fma(C.w.x, west0, fma(C.e.x, c.y, c.x))));
-  o.y = fma(C.s.y, m.y, fma(C.n.y, n.y, fma(C.w.y, c.x, fma(C.e.y, east1, c.y))));
+  o.x = fma(C.s[0], m.x, fma(C.n[0], n.x, fma(C.w[0], west0, C.e[0] * c.y)));
+  o.y = fma(C.s[1], m.y, fma(C.n[1], n.y, fma(C.w[1], c.x, C.e[1] * east1)));
   return o;
 }
 
-// Operand requests per sweep step (measured on config 5, 8192 x 8192, us per iteration: old
-// load-at-use order 2297; B prefetched + CA grouped 2069; both prefetched 2447 (CA's second operand
-// set spills); both passes out of line 2611 (the parameter block then lives in local memory);
-// cp.async rings in shared memory, 2 or 3 rows deep, 2362 / 2443; t recomputed in pass CA instead
-// of stored by pass B and read back, 20 instead of 22 doubles per node-iteration, 2165 (its extra
-// live rows spill at 128 registers; 2271 with 192-thread CTAs and 168 registers)).
-constexpr bool PF_B = true;    // pass B: request the next step's operands before computing this one
-constexpr bool PF_CA = false;  // pass CA: all ten operand loads of a step up front, then compute
-#ifndef NH_DEFER_CA
-#define NH_DEFER_CA 1
-#endif
-constexpr bool DEFER_CA = NH_DEFER_CA;  // pass CA: next step's loads issued before this step's stores
+// Every pass is software-pipelined by hand: the loads of the NEXT row are issued before the current
+// row is computed and stored (the compiler cannot hoist them itself across the stores of possibly
+// aliasing planes), so each warp keeps one full row of every plane in flight while it computes.
 
-// pass B: s = r - alpha v (rows Ja-1..Jb), t = (A M^-1) s (rows Ja..Jb-1);
-// partials: t.s, t.t, s.s, r0.s, r0.t
-struct RowB {  // operands of one sweep step of pass B: vectors of row j+1, coefficients of row j
-  double2 r, v;
-  RowC C;
+// residual pass: r = b - A x (S9: the true residual decides), r0 = r, r^ = r / A_C; partials r.r, b.b
+__device__ __forceinline__ void pass_R(const SolveP& P, double* rh, int buf, double (*red)[NW]) {
+  const NhGrid& G = P.G;
+  const int lane = threadIdx.x & 31;
+  const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
+  const int nunits = P.nstrips * P.nbands;
+  double acc[2] = {0.0, 0.0};
+  for (int k = gw; k < nunits; k += tw) {
+    Unit U = make_unit(P, k, lane);
+    March M;
+    M.start(P, U.c0, U.Ja);
+    double2 xm = ld2(P.x, G, U.c0, U.Ja - 1), xc = ld2(P.x, G, U.c0, U.Ja);
+    for (int j = U.Ja; j < U.Jb; ++j) {
+      const double2 xn = ld2(P.x, G, U.c0, j + 1), bb = ld2(P.b, G, U.c0, j);
+      const Coef C = M.step(P, ld2(P.hc, G, U.c0, j), ld2(P.zc, G, U.c0, j + 1));
+      const double2 off = offdiag2(C, xm, xc, xn);
+      const double2 rr = make_double2(bb.x - fma(C.c[0], xc.x, off.x), bb.y - fma(C.c[1], xc.y, off.y));
+      st2(P.r0, P, U, j, rr);
+      st2(rh, P, U, j, make_double2(rr.x * rcp_diag(C.c[0]), rr.y * rcp_diag(C.c[1])));
+      if (U.own0) { acc[0] = fma(rr.x, rr.x, acc[0]); acc[1] = fma(bb.x, bb.x, acc[1]); }
+      if (U.own1) { acc[0] = fma(rr.y, rr.y, acc[0]); acc[1] = fma(bb.y, bb.y, acc[1]); }
+      xm = xc; xc = xn;
+    }
+  }
+  block_partials<2>(acc, P.part, buf, red);
+}
+
+// pass B: s^ = r^ - alpha v^ (rows Ja-1..Jb), t = A s^ (rows Ja..Jb-1), stored as t^ = t / A_C;
+// partials of the unscaled vectors: t.s, t.t, s.s, r0.s, r0.t
+struct RowB {  // operands of sweep step j: r^, v^ of row j+1; r0, h of row j; z of row j+1
+  double2 r, v, q, h, z;
 };
 __device__ __forceinline__ void ld_rowb(RowB& X, const SolveP& P, const double* r, const double* v,
-                                        int c0, int jv, int jc) {
-  X.r = ld2(r, P.G, c0, jv); X.v = ld2(v, P.G, c0, jv);
-  X.C = ld_rowc(P, c0, jc);
+                                        int c0, int j) {
+  X.r = ld2(r, P.G, c0, j + 1); X.v = ld2(v, P.G, c0, j + 1);
+  X.q = ld2(P.r0, P.G, c0, j);
+  X.h = ld2(P.hc, P.G, c0, j); X.z = ld2(P.zc, P.G, c0, j + 1);
 }
 
 __device__ __forceinline__ void pass_B(const SolveP& P, double alpha, const double* r, const double* v,
@@ -241,46 +338,48 @@ __device__ __forceinline__ void pass_B(const SolveP& P, double alpha, const doub
   const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
   const int nunits = P.nstrips * P.nbands;
   double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-  for (int u = gw; u < nunits; u += tw) {
-    Unit U = make_unit(P, u, lane);
+  for (int k = gw; k < nunits; k += tw) {
+    Unit U = make_unit(P, k, lane);
     auto srow = [&](double2 a, double2 b) {
       return make_double2(fma(-alpha, b.x, a.x), fma(-alpha, b.y, a.y));
     };
+    March M;
+    M.start(P, U.c0, U.Ja);
     double2 sm = srow(ld2(r, G, U.c0, U.Ja - 1), ld2(v, G, U.c0, U.Ja - 1));
     double2 sc = srow(ld2(r, G, U.c0, U.Ja), ld2(v, G, U.c0, U.Ja));
-    // one sweep step: row j from the operand set `cur`; the set of the next step is requested
-    // first (`nxt`; row indices clamped, the last request is never used)
-    auto step = [&](int j, RowB& cur, RowB& nxt) {
-      if (PF_B) ld_rowb(nxt, P, r, v, U.c0, min(j + 2, U.Jb), min(j + 1, U.Jb - 1));
-      else ld_rowb(cur, P, r, v, U.c0, j + 1, j);
-      double2 sn = srow(cur.r, cur.v);
-      double2 t = stencil2(cur.C, sm, sc, sn);
-      st2(P.t, P, U, j, t);
-      const double2 q = cur.C.q;
+    // One operand set; the loads of step j+1 are issued as soon as step j has moved its operands
+    // into the marching state, before the arithmetic of the step (row index clamped: the last
+    // request is never used).
+    RowB X;
+    ld_rowb(X, P, r, v, U.c0, U.Ja);
+    for (int j = U.Ja; j < U.Jb; ++j) {
+      const double2 sn = srow(X.r, X.v);
+      const double2 q = X.q;
+      const Coef C = M.step(P, X.h, X.z);
+      if (j + 1 < U.Jb) ld_rowb(X, P, r, v, U.c0, j + 1);
+      const double2 off = offdiag2(C, sm, sc, sn);
+      const double2 tu = make_double2(fma(C.c[0], sc.x, off.x), fma(C.c[1], sc.y, off.y));  // t
+      const double2 su = make_double2(C.c[0] * sc.x, C.c[1] * sc.y);                        // s
+      st2(P.t, P, U, j, make_double2(fma(rcp_diag(C.c[0]), off.x, sc.x), fma(rcp_diag(C.c[1]), off.y, sc.y)));
       if (U.own0) {
-        acc[0] = fma(t.x, sc.x, acc[0]); acc[1] = fma(t.x, t.x, acc[1]); acc[2] = fma(sc.x, sc.x, acc[2]);
-        acc[3] = fma(q.x, sc.x, acc[3]); acc[4] = fma(q.x, t.x, acc[4]);
+        acc[0] = fma(tu.x, su.x, acc[0]); acc[1] = fma(tu.x, tu.x, acc[1]); acc[2] = fma(su.x, su.x, acc[2]);
+        acc[3] = fma(q.x, su.x, acc[3]); acc[4] = fma(q.x, tu.x, acc[4]);
       }
       if (U.own1) {
-        acc[0] = fma(t.y, sc.y, acc[0]); acc[1] = fma(t.y, t.y, acc[1]); acc[2] = fma(sc.y, sc.y, acc[2]);
-        acc[3] = fma(q.y, sc.y, acc[3]); acc[4] = fma(q.y, t.y, acc[4]);
+        acc[0] = fma(tu.y, su.y, acc[0]); acc[1] = fma(tu.y, tu.y, acc[1]); acc[2] = fma(su.y, su.y, acc[2]);
+        acc[3] = fma(q.y, su.y, acc[3]); acc[4] = fma(q.y, tu.y, acc[4]);
       }
       sm = sc; sc = sn;
-    };
-    RowB A, B;
-    if (PF_B) ld_rowb(A, P, r, v, U.c0, U.Ja + 1, U.Ja);
-    for (int j = U.Ja; j < U.Jb; j += 2) {  // ping-pong operand sets: no register rotation
-      step(j, A, B);
-      if (j + 1 < U.Jb) step(j + 1, B, A);
     }
   }
   block_partials<5>(acc, P.part, buf, red);
 }
 
-// pass CA: FIRST: p' = r' = r (start of a cycle).  Otherwise s = r - alpha v; y += alpha p + omega s;
-// r' = s - omega t; p' = r' + beta (p - omega v).  Then v' = (A M^-1) p'.  partials: r0.v', r'.r'
+// pass CA: FIRST: p^' = r^' = r^ (start of a cycle).  Otherwise s^ = r^ - alpha v^;
+// x += alpha p^ + omega s^; r^' = s^ - omega t^; p^' = r^' + beta (p^ - omega v^).  Then v' = A p^',
+// stored as v^' = v' / A_C.  partials of the unscaled vectors: r0.v', r'.r'
 struct RowV {  // vector row of pass CA
-  double2 r, v, t, p, y;
+  double2 r, v, t, p, x;
 };
 template <bool FIRST>
 __device__ __forceinline__ void ld_rowv(RowV& V, const SolveP& P, const double* r, const double* p,
@@ -288,12 +387,12 @@ __device__ __forceinline__ void ld_rowv(RowV& V, const SolveP& P, const double* 
   V.r = ld2(r, P.G, c0, j);
   if (!FIRST) {
     V.v = ld2(v, P.G, c0, j); V.t = ld2(P.t, P.G, c0, j);
-    V.p = ld2(p, P.G, c0, j); V.y = ld2(P.y, P.G, c0, j);
+    V.p = ld2(p, P.G, c0, j); V.x = ld2(P.x, P.G, c0, j);
   }
 }
-struct RowCA {  // operands of one sweep step of pass CA: vectors of row j+1, coefficients of row j
+struct RowCA {  // operands of sweep step j: vectors of row j+1; r0, h of row j; z of row j+1
   RowV V;
-  RowC C;
+  double2 q, h, z;
 };
 
 template <bool FIRST>
@@ -304,152 +403,95 @@ __device__ __forceinline__ void pass_CA(const SolveP& P, double alpha, double om
   const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
   const int nunits = P.nstrips * P.nbands;
   double acc[2] = {0.0, 0.0};
-  for (int u = gw; u < nunits; u += tw) {
-    Unit U = make_unit(P, u, lane);
-    // new p of row j from its loaded operands; on owned rows also the y / r' / p' stores and the
-    // r'.r' partial
-    auto prow = [&](const RowV& V, int j, bool owned_row) {
-      double2 rn, pn;
+  for (int k = gw; k < nunits; k += tw) {
+    Unit U = make_unit(P, k, lane);
+    // new r^, p^, x of a row from its loaded operands
+    auto vrow = [&](const RowV& V, double2& rn, double2& pn, double2& xx) {
       if (FIRST) {
-        rn = V.r; pn = V.r;
+        rn = V.r; pn = V.r; xx = V.r;
       } else {
-        double2 s = make_double2(fma(-alpha, V.v.x, V.r.x), fma(-alpha, V.v.y, V.r.y));
+        const double2 s = make_double2(fma(-alpha, V.v.x, V.r.x), fma(-alpha, V.v.y, V.r.y));
         rn = make_double2(fma(-omega, V.t.x, s.x), fma(-omega, V.t.y, s.y));
         pn = make_double2(fma(beta, fma(-omega, V.v.x, V.p.x), rn.x),
                           fma(beta, fma(-omega, V.v.y, V.p.y), rn.y));
-        if (owned_row) {
-          double2 yy;
-          yy.x = V.y.x + fma(omega, s.x, alpha * V.p.x);
-          yy.y = V.y.y + fma(omega, s.y, alpha * V.p.y);
-          st2(P.y, P, U, j, yy);
-        }
+        xx = make_double2(V.x.x + fma(omega, s.x, alpha * V.p.x), V.x.y + fma(omega, s.y, alpha * V.p.y));
       }
-      if (owned_row) {
-        st2(rN, P, U, j, rn);
-        st2(pN, P, U, j, pn);
-        if (U.own0) acc[1] = fma(rn.x, rn.x, acc[1]);
-        if (U.own1) acc[1] = fma(rn.y, rn.y, acc[1]);
-      }
-      return pn;
     };
-    double2 pm, pc;
+    auto store_row = [&](int j, double2 rn, double2 pn, double2 xx) {
+      if (!FIRST) st2(P.x, P, U, j, xx);
+      st2(rN, P, U, j, rn);
+      st2(pN, P, U, j, pn);
+    };
+    auto ld_set = [&](RowCA& X, int j) {
+      ld_rowv<FIRST>(X.V, P, r, p, v, U.c0, j + 1);
+      X.q = ld2(P.r0, P.G, U.c0, j);
+      X.h = ld2(P.hc, P.G, U.c0, j); X.z = ld2(P.zc, P.G, U.c0, j + 1);
+    };
+    March M;
+    M.start(P, U.c0, U.Ja);
+    double2 pm, pc, rc;  // p^' of rows j-1, j; r^' of row j (its A_C is known one step later)
     {
       RowV V0, V1;
       ld_rowv<FIRST>(V0, P, r, p, v, U.c0, U.Ja - 1);
       ld_rowv<FIRST>(V1, P, r, p, v, U.c0, U.Ja);
-      pm = prow(V0, U.Ja - 1, false);
-      pc = prow(V1, U.Ja, true);
+      double2 r0_, x0_, x1_;
+      vrow(V0, r0_, pm, x0_);
+      vrow(V1, rc, pc, x1_);
+      store_row(U.Ja, rc, pc, x1_);
     }
-    auto ld_set = [&](RowCA& X, int jv, int jc) {
-      ld_rowv<FIRST>(X.V, P, r, p, v, U.c0, jv);
-      X.C = ld_rowc(P, U.c0, jc);
-    };
-    auto step = [&](int j, RowCA& cur, RowCA& nxt) {
-      if (PF_CA) ld_set(nxt, min(j + 2, U.Jb), min(j + 1, U.Jb - 1));
-      else ld_set(cur, j + 1, j);
-      double2 pn = prow(cur.V, j + 1, j + 1 < U.Jb);
-      double2 vv = stencil2(cur.C, pm, pc, pn);
-      st2(vN, P, U, j, vv);
-      if (U.own0) acc[0] = fma(cur.C.q.x, vv.x, acc[0]);
-      if (U.own1) acc[0] = fma(cur.C.q.y, vv.y, acc[0]);
-      pm = pc; pc = pn;
-    };
-    if (!FIRST && DEFER_CA) {
-      // One operand set; the loads of step j+1 are issued as soon as step j has consumed its
-      // operands, BEFORE its four stores (ghost-image logic included) and its dot-product terms,
-      // which then run in the shadow of the memory latency.
-      RowCA X;
-      ld_set(X, U.Ja + 1, U.Ja);
-      for (int j = U.Ja; j < U.Jb; ++j) {
-        const RowV& V = X.V;
-        const bool own_next = j + 1 < U.Jb;
-        double2 sv = make_double2(fma(-alpha, V.v.x, V.r.x), fma(-alpha, V.v.y, V.r.y));
-        double2 rn = make_double2(fma(-omega, V.t.x, sv.x), fma(-omega, V.t.y, sv.y));
-        double2 pn = make_double2(fma(beta, fma(-omega, V.v.x, V.p.x), rn.x),
-                                  fma(beta, fma(-omega, V.v.y, V.p.y), rn.y));
-        double2 yy = make_double2(V.y.x + fma(omega, sv.x, alpha * V.p.x),
-                                  V.y.y + fma(omega, sv.y, alpha * V.p.y));
-        double2 vv = stencil2(X.C, pm, pc, pn);
-        const double2 q = X.C.q;
-        if (own_next) ld_set(X, min(j + 2, U.Jb), j + 1);  // operands of the next step
-        if (own_next) {
-          st2(P.y, P, U, j + 1, yy);
-          st2(rN, P, U, j + 1, rn);
-          st2(pN, P, U, j + 1, pn);
-          if (U.own0) acc[1] = fma(rn.x, rn.x, acc[1]);
-          if (U.own1) acc[1] = fma(rn.y, rn.y, acc[1]);
-        }
-        st2(vN, P, U, j, vv);
-        if (U.own0) acc[0] = fma(q.x, vv.x, acc[0]);
-        if (U.own1) acc[0] = fma(q.y, vv.y, acc[0]);
-        pm = pc; pc = pn;
-      }
-    } else {
-      RowCA A, B;
-      if (PF_CA) ld_set(A, U.Ja + 1, U.Ja);
-      for (int j = U.Ja; j < U.Jb; j += 2) {  // ping-pong operand sets: no register rotation
-        step(j, A, B);
-        if (j + 1 < U.Jb) step(j + 1, B, A);
-      }
+    // One operand set; the loads of step j+1 are issued as soon as step j has consumed its operands,
+    // BEFORE its stores (ghost-image logic included) and its dot-product terms, which then run in
+    // the shadow of the memory latency.
+    RowCA X;
+    ld_set(X, U.Ja);
+    for (int j = U.Ja; j < U.Jb; ++j) {
+      const bool own_next = j + 1 < U.Jb;
+      double2 rn, pn, xx;
+      vrow(X.V, rn, pn, xx);
+      const Coef C = M.step(P, X.h, X.z);
+      const double2 q = X.q;
+      if (own_next) ld_set(X, min(j + 1, U.Jb - 1));  // operands of the next step
+      const double2 off = offdiag2(C, pm, pc, pn);
+      const double2 vu = make_double2(fma(C.c[0], pc.x, off.x), fma(C.c[1], pc.y, off.y));  // v'
+      if (own_next) store_row(j + 1, rn, pn, xx);
+      st2(vN, P, U, j, make_double2(fma(rcp_diag(C.c[0]), off.x, pc.x), fma(rcp_diag(C.c[1]), off.y, pc.y)));
+      const double2 ru = make_double2(C.c[0] * rc.x, C.c[1] * rc.y);  // r' of row j
+      if (U.own0) { acc[0] = fma(q.x, vu.x, acc[0]); acc[1] = fma(ru.x, ru.x, acc[1]); }
+      if (U.own1) { acc[0] = fma(q.y, vu.y, acc[0]); acc[1] = fma(ru.y, ru.y, acc[1]); }
+      pm = pc; pc = pn; rc = rn;
     }
   }
   block_partials<2>(acc, P.part, buf, red);
 }
 
 // ---- simple phases (a handful per solve): rows over CTAs, columns over threads --------------
-// y = dg * x at the real nodes, with ghost images
-__device__ void phase_y_from_x(const SolveP& P) {
+// ghost images of the start vector
+__device__ void phase_images(const SolveP& P) {
   const NhGrid& G = P.G;
   for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
-    for (int I = threadIdx.x; I < G.nnx; I += NT) {
-      size_t k = nidx(G, I, J);
-      store_images(G, P.y, I, J, P.x[k] * P.dg[k]);
-    }
+    for (int I = threadIdx.x; I < G.nnx; I += NT) store_images(G, P.x, I, J, P.x[nidx(G, I, J)]);
 }
 
-// true residual r = b - (A M^-1) y, r0 = r (S9: the true residual decides); partials r.r, b.b
-__device__ void phase_init(const SolveP& P, double* r, int buf, double (*red)[NW]) {
-  const NhGrid& G = P.G;
-  double acc[2] = {0.0, 0.0};
-  for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
-    for (int I = threadIdx.x; I < G.nnx; I += NT) {
-      size_t k = nidx(G, I, J);
-      const double* y = P.y;
-      double ay = y[k] + P.cE[k] * y[k + 1] + P.cW[k] * y[k - 1] + P.cN[k] * y[k + G.np] +
-                  P.cS[k] * y[k - G.np];
-      double bb = P.b[k];
-      double rr = bb - ay;
-      store_images(G, r, I, J, rr);
-      P.r0[k] = rr;
-      acc[0] += rr * rr; acc[1] += bb * bb;
-    }
-  block_partials<2>(acc, P.part, buf, red);
-}
-
-// y += alpha p + omega s, s = r - alpha v  (final update of an iteration whose pass CA never ran:
-// half-step exit with omega = 0, and the polish iteration)
-__device__ void phase_update_y(const SolveP& P, double alpha, double omega, const double* r,
+// x += alpha p^ + omega s^, s^ = r^ - alpha v^  (final update of an iteration whose pass CA never
+// ran: half-step exit with omega = 0, and the polish iteration)
+__device__ void phase_update_x(const SolveP& P, double alpha, double omega, const double* r,
                                const double* p, const double* v) {
   const NhGrid& G = P.G;
   for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
     for (int I = threadIdx.x; I < G.nnx; I += NT) {
       size_t k = nidx(G, I, J);
       double s = r[k] - alpha * v[k];
-      store_images(G, P.y, I, J, P.y[k] + (alpha * p[k] + omega * s));
+      store_images(G, P.x, I, J, P.x[k] + (alpha * p[k] + omega * s));
     }
 }
 
-// x = M^-1 y  (or zeros when b = 0)
-__device__ void phase_out(const SolveP& P, bool zero) {
+__device__ void phase_zero_x(const SolveP& P) {
   const NhGrid& G = P.G;
   for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
-    for (int I = threadIdx.x; I < G.nnx; I += NT) {
-      size_t k = nidx(G, I, J);
-      P.x[k] = zero ? 0.0 : P.y[k] * P.dinv[k];
-    }
+    for (int I = threadIdx.x; I < G.nnx; I += NT) store_images(G, P.x, I, J, 0.0);
 }
 
-__global__ void __launch_bounds__(NT, 2) k_bicgstab(SolveP P) {
+__global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
   cg::grid_group grid = cg::this_grid();
   __shared__ double red[MAXDOT][NW];
   __shared__ double bc[MAXDOT];
@@ -465,11 +507,11 @@ __global__ void __launch_bounds__(NT, 2) k_bicgstab(SolveP P) {
   int iters = 0, converged = 0, status = 0;
   double rnorm = 0.0, bnorm = 0.0, tol = 0.0;
 
-  phase_y_from_x(P);
+  phase_images(P);
   grid.sync();
   for (int cycle = 0; cycle < 8 && !converged; ++cycle) {
     double d2[2], d5[5];
-    phase_init(P, rC, buf, red);
+    pass_R(P, rC, buf, red);
     grid.sync();
     grid_sums<2>(P.part, buf, d2, red, bc);
     buf ^= 1;
@@ -483,7 +525,7 @@ __global__ void __launch_bounds__(NT, 2) k_bicgstab(SolveP P) {
     if (!(rnorm == rnorm)) { status = NH_ENAN; break; }
     if (rnorm <= tol) { converged = 1; break; }
     if (iters >= P.maxit) break;
-    // first direction of the cycle: p = r, v = (A M^-1) p, sigma = r0.v
+    // first direction of the cycle: p = r, v = A M^-1 p, sigma = r0.v
     double rho = d2[0];
     pass_CA<true>(P, 0.0, 0.0, 0.0, rC, pC, vC, rN, pN, vN, buf, red);
     flip();
@@ -500,7 +542,7 @@ __global__ void __launch_bounds__(NT, 2) k_bicgstab(SolveP P) {
       grid_sums<5>(P.part, buf, d5, red, bc);
       buf ^= 1;
       if (sqrt(d5[2]) <= tol) {  // half-step exit: x += alpha p^
-        phase_update_y(P, alpha, 0.0, rC, pC, vC);
+        phase_update_x(P, alpha, 0.0, rC, pC, vC);
         grid.sync();
         break;
       }
@@ -541,11 +583,11 @@ __global__ void __launch_bounds__(NT, 2) k_bicgstab(SolveP P) {
       grid_sums<5>(P.part, buf, d5, red, bc);
       buf ^= 1;
       double omega = (d5[1] > 0.0) ? d5[0] / d5[1] : 0.0;
-      phase_update_y(P, alpha, omega, rC, pC, vC);
+      phase_update_x(P, alpha, omega, rC, pC, vC);
       grid.sync();
     }
   }
-  if (status != NH_ENAN) phase_out(P, bnorm == 0.0);
+  if (status != NH_ENAN && bnorm == 0.0) phase_zero_x(P);  // b = 0 => p~ = 0, zero iterations
 
   if (blockIdx.x == 0 && threadIdx.x == 0) {
     NhScal* sc = P.sc;
@@ -569,6 +611,7 @@ __global__ void __launch_bounds__(NT, 2) k_bicgstab(SolveP P) {
 // order the oracle uses (no FMA), a max is exact, and a Jacobi sweep does not depend on the sweep
 // order: the iterates, the iteration count and E are bit-identical to the CPU oracle's.
 // Traffic: reads x, b', 4 c; writes x': 7 doubles = 56 B per node-iteration.
+constexpr int NT1 = 256, NW1 = NT1 / 32;  // CTA shape of k_srj (128 registers, 16 warps per SM)
 struct SrjP {
   NhGrid G;
   int nstrips, R, nbands;
@@ -583,7 +626,7 @@ __device__ __forceinline__ void srj_sweep(const SrjP& P, const SolveP& Q, double
                                           double* xn, unsigned long long* Eslot) {
   const NhGrid& G = P.G;
   const int lane = threadIdx.x & 31;
-  const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
+  const int gw = blockIdx.x * NW1 + (threadIdx.x >> 5), tw = gridDim.x * NW1;
   const int nunits = P.nstrips * P.nbands;
   double emax = 0.0;
   bool bad = false;
@@ -619,13 +662,13 @@ __device__ __forceinline__ void srj_sweep(const SrjP& P, const SolveP& Q, double
   }
   // CTA max -> one integer atomicMax (exact, order independent)
   for (int o = 16; o > 0; o >>= 1) emax = fmax(emax, __shfl_xor_sync(0xffffffffu, emax, o));
-  __shared__ double wmax[NW];
+  __shared__ double wmax[NW1];
   if (lane == 0) wmax[threadIdx.x >> 5] = emax;
   int anybad = __syncthreads_or(bad);
   if (threadIdx.x == 0) {
     double m = 0.0;
 #pragma unroll
-    for (int w = 0; w < NW; ++w) m = fmax(m, wmax[w]);
+    for (int w = 0; w < NW1; ++w) m = fmax(m, wmax[w]);
     if (m > 0.0) atomicMax(Eslot, (unsigned long long)__double_as_longlong(m));
     if (anybad) atomicOr(&P.sc->srj_bad, 1);
   }
@@ -634,7 +677,7 @@ __device__ __forceinline__ void srj_sweep(const SrjP& P, const SolveP& Q, double
 #ifndef NH_SRJ_MINB
 #define NH_SRJ_MINB 2
 #endif
-__global__ void __launch_bounds__(NT, NH_SRJ_MINB) k_srj(SrjP P) {
+__global__ void __launch_bounds__(NT1, NH_SRJ_MINB) k_srj(SrjP P) {
   cg::grid_group grid = cg::this_grid();
   const NhGrid& G = P.G;
   NhScal* sc = P.sc;
@@ -649,7 +692,7 @@ __global__ void __launch_bounds__(NT, NH_SRJ_MINB) k_srj(SrjP P) {
     status = NH_ENAN;
   } else if (bmax == 0.0) {  // b = 0 => p~ = 0, zero iterations (same convention as solver 0)
     for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
-      for (int I = threadIdx.x; I < G.nnx; I += NT) P.xA[nidx(G, I, J)] = 0.0;
+      for (int I = threadIdx.x; I < G.nnx; I += NT1) P.xA[nidx(G, I, J)] = 0.0;
   } else {
     // cycle length: smallest power of two with M sqrt(2 (1 - rho)) >= 7.6, at most mmax.  Where a
     // row is not strictly diagonally dominant (rho >= 1, e.g. across a discontinuous free surface)
@@ -663,7 +706,7 @@ __global__ void __launch_bounds__(NT, NH_SRJ_MINB) k_srj(SrjP P) {
     const double tol = (P.rel > 0.0) ? P.rel * bmax : P.eps;
     // ghost images of the start vector
     for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
-      for (int I = threadIdx.x; I < G.nnx; I += NT) store_images(G, x, I, J, x[nidx(G, I, J)]);
+      for (int I = threadIdx.x; I < G.nnx; I += NT1) store_images(G, x, I, J, x[nidx(G, I, J)]);
     grid.sync();
     for (;;) {
       const double om = dominant ? 1.0 / (1.0 - rho * cosv[iters % M]) : 1.0;
@@ -681,7 +724,7 @@ __global__ void __launch_bounds__(NT, NH_SRJ_MINB) k_srj(SrjP P) {
     }
     if (x != P.xA) {  // the accepted iterate lives in the scratch plane
       for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
-        for (int I = threadIdx.x; I < G.nnx; I += NT) P.xA[nidx(G, I, J)] = x[nidx(G, I, J)];
+        for (int I = threadIdx.x; I < G.nnx; I += NT1) P.xA[nidx(G, I, J)] = x[nidx(G, I, J)];
     }
   }
   grid.sync();
@@ -742,15 +785,15 @@ int nh_solver_setup(nh_ctx* c) {
     // cos(pi (2 perm_i - 1) / 2M) in Lebedev-Finogenov order for M = 1, 2, 4, ..., mmax (R28),
     // evaluated on the host so that the factors are the ones a CPU evaluation produces.
     int occ1 = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_srj, NT, 0);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_srj, NT1, 0);
     if (e != cudaSuccess || occ1 < 1) {
       snprintf(c->err, sizeof(c->err), "srj occupancy query failed: %s", cudaGetErrorString(e));
       return NH_ECUDA;
     }
     long long g1 = (long long)occ1 * c->sm_count;
-    if (g1 > (small_units + NW - 1) / NW) g1 = (small_units + NW - 1) / NW;
+    if (g1 > (small_units + NW1 - 1) / NW1) g1 = (small_units + NW1 - 1) / NW1;
     if (g1 < 1) g1 = 1;
-    const long long tw1 = g1 * NW;
+    const long long tw1 = g1 * NW1;
     int R1 = nny;
     long long best1 = -1;
     for (int R = 4; R <= nny; ++R) {
@@ -791,7 +834,7 @@ void nh_launch_solve(nh_ctx* c, const double* b, double* x, int count_stats) {
     S.xA = x; S.xB = c->ky; S.sc = c->sc; S.eps = c->prm.srj_eps; S.rel = c->prm.srj_rel;
     S.maxit = c->prm.solver_maxit; S.mmax = c->prm.srj_mmax; S.count_stats = count_stats;
     void* args[] = {&S};
-    NH_CUDA_OK(c, cudaLaunchCooperativeKernel((void*)k_srj, dim3(c->srj_grid), dim3(NT), args, 0,
+    NH_CUDA_OK(c, cudaLaunchCooperativeKernel((void*)k_srj, dim3(c->srj_grid), dim3(NT1), args, 0,
                                               c->stream));
     c->launches++;
     return;
@@ -799,11 +842,12 @@ void nh_launch_solve(nh_ctx* c, const double* b, double* x, int count_stats) {
   SolveP P;
   P.G = c->g;
   P.nstrips = c->solver_nstrips; P.R = c->solver_R; P.nbands = c->solver_nbands;
-  P.cE = c->cE; P.cW = c->cW; P.cN = c->cN; P.cS = c->cS; P.dg = c->dg; P.dinv = c->dinv;
+  P.hc = c->hc; P.zc = c->zc;
   P.b = b; P.x = x;
-  P.y = c->ky; P.r0 = c->kr0; P.t = c->kt;
+  P.r0 = c->kr0; P.t = c->kt;
   P.rA = c->kr; P.rB = c->krB; P.pA = c->kpA; P.pB = c->kpB; P.vA = c->kvA; P.vB = c->kvB;
   P.part = c->part; P.sc = c->sc; P.rtol = c->prm.solver_rtol; P.maxit = c->prm.solver_maxit;
+  P.miex = -1.0 / (8.0 * c->g.dx * c->g.dx); P.miey = -1.0 / (8.0 * c->g.dy * c->g.dy);
   P.count_stats = count_stats;
   void* args[] = {&P};
   NH_CUDA_OK(c, cudaLaunchCooperativeKernel((void*)k_bicgstab, dim3(c->solver_grid), dim3(NT), args,

@@ -4,7 +4,8 @@ This module holds NONE of the method's arithmetic: it only builds bathymetry H, 
 (h, qx, qy, w, p) arrays and the parameter dictionaries of the five BASELINE.json configs
 (restated in SURVEY.md 8(d) / DESIGN.md "Input recipe").  No public dataset is used: the
 configs stand in for the paper's workloads (1D solitary channel PAPER.md L552-560,
-Synolakis-type beach L623-635, 2D basin L669-677, dam-break grids L700-720).
+Synolakis-type beach L623-635, 2D basin L669-677, dam-break grids L700-720); `conical_island` is the
+geometry of the paper's section 7.6 (L669-677) as a second synthetic workload.
 
 Arrays are NumPy float64, cell fields (ny, nx), node fields (ny+1, nx+1), C order (x fastest).
 Every generator takes the grid size so tests can run the same recipe on smaller grids.
@@ -185,6 +186,34 @@ def paper_dam_break(n=250):
     params = dict(g=9.81, cfl=0.9, nonhydro=1, breaking=0, time_order=2,
                   bc_xlo=BC_OUTFLOW, bc_xhi=BC_OUTFLOW, bc_ylo=BC_OUTFLOW, bc_yhi=BC_OUTFLOW)
     return _pack("paper_dam_break", n, n, dx, dx, H, h, 0.0, 0.0, params, 1.25, int(0.8 * n))
+
+
+def conical_island(n=1400, w_advect=0):
+    """The geometry of the paper's second 2D workload (section 7.6): basin
+    [-5, 23] x [0, 28] m at still-water depth 0.32 m with a conical island (base diameter 7.2 m, top
+    diameter 2.2 m, 0.625 m high, side slope 1:4) whose top emerges; solitary wave (33) of amplitude
+    0.06 m centred at x = 0 for eta and u; Manning n = 0.015, breaking with B1 = 0.15, B2 = 0.5,
+    CFL 0.9, free outflow on all sides.  n x n cells (the paper: dx = 2 cm, n = 1400); the island
+    sits at the centre of the numerical domain (the text says "near the center"; the gauge positions
+    and the laboratory records are not used).  Geometry and formulas only -- a synthetic stand-in,
+    compared between the oracle and the CUDA path, never against the measurements.  `steps` is the
+    step count to t = 30 s at the paper's resolution, scaled with n."""
+    g, H0, A = 9.81, 0.32, 0.06
+    dx = 28.0 / n
+    x = (np.arange(n) + 0.5) * dx - 5.0
+    y = (np.arange(n) + 0.5) * dx
+    X, Y = np.meshgrid(x, y)
+    r = np.sqrt((X - 9.0) ** 2 + (Y - 14.0) ** 2)
+    zb = np.clip(0.25 * (3.6 - r), 0.0, 0.625)          # bed above the basin floor: cone frustum
+    H = H0 - zb
+    eta = A / np.cosh(np.sqrt(3.0 * A / (4.0 * H0 ** 3)) * X) ** 2
+    h = np.maximum(H + eta, 0.0)
+    c = np.sqrt(g * (H0 + A))
+    qx = np.where(h > 0.0, c * eta, 0.0)
+    params = dict(g=g, cfl=0.9, nonhydro=1, breaking=1, B1=0.15, B2=0.5, manning_n=0.015, time_order=2,
+                  w_advect=int(w_advect),
+                  bc_xlo=BC_OUTFLOW, bc_xhi=BC_OUTFLOW, bc_ylo=BC_OUTFLOW, bc_yhi=BC_OUTFLOW)
+    return _pack("conical_island", n, n, dx, dx, H, h, qx, 0.0, params, H0, int(7.0 * n))
 
 
 CONFIGS = {1: config1_channel, 2: config2_lake, 3: config3_radial, 4: config4_beach,

@@ -56,36 +56,54 @@ def test_config3_radial_hump_500_steps(O, G):
 
 
 def test_config4_beach_2000_steps_narrow(O, G):
-    # the whole configured run of config 4 -- generation, shoaling, breaking, run-up over the dry
-    # slope and plateau -- on a 640 x 8 strip of the same beach (same dx, slope, y-perturbed bed,
-    # generating zone, breaking and wet/dry parameters); the bore overtops the +0.2 m plateau and a
-    # thin film runs over the dry bed to the wall: the negative-depth clamp of R7 acts on real values
+    """The whole configured run of config 4 -- generation, shoaling, breaking, run-up over the dry slope
+    and plateau -- on a 640 x 8 strip of the same beach (same dx, slope, y-perturbed bed, generating
+    zone, breaking and wet/dry parameters); the bore overtops the +0.2 m plateau and a thin film runs
+    over the dry bed to the wall: the negative-depth clamp of R7 acts on real values.
+
+    This run is SENSITIVE: the breaking switch (9) and the wet/dry front turn differences of the
+    size of the solver tolerance into O(1e-3) differences (two ORACLE runs at solver_rtol 1e-12 and
+    1e-13 differ by 1e4 bars right after breaking sets in and by 4e6 bars at step 2000,
+    profiles/r02b_config4_sensitivity.md), so an element-by-element bar over the full horizon is only
+    meaningful where both sides do the same arithmetic: with the paper's solver (solver 1, R28) the
+    CUDA path reproduces the oracle BIT FOR BIT through all 2000 steps.  The default solver is then
+    held against the same oracle run by what is unique: the wet/dry front, the run-up, the breaking
+    activity, and the state within the spread two valid solves show."""
     cfg = inputs.make_config(4, nx=640, ny=8)
     assert cfg["steps"] == 2000 and cfg["params"]["breaking"] == 1
     wet0 = cfg["h"] > 1e-5
-    o, g = both(O, G, cfg)
+    o, g = both(O, G, cfg, solver=1, srj_eps=1e-6)
+    g0 = G.NH(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["H"], **cfg["params"])   # default solver
+    g0.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
     probe = O.Oracle(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["H"], **cfg["params"])
     done, broke, wet_max = 0, 0, 0
     for k in range(10):
         o.step(200)
         g.step(200)
+        g0.step(200)
         done += 200
-        assert g.sync() == 0
-        so, sg = o.get_state(), g.get_state()
-        r = parity(sg, so, cfg["H"], cfg["h0"])
-        assert all(np.isfinite(v) and v <= 1.0 for v in r.values()), (done, r)
-        assert np.array_equal(sg["h"] > 1e-5, so["h"] > 1e-5)        # the same wet/dry front
-        wet_max = max(wet_max, int(np.sum((so["h"] > 1e-5) & ~wet0)))
+        assert g.sync() == 0 and g0.sync() == 0
+        so, sg, s0 = o.get_state(), g.get_state(), g0.get_state()
+        for f in ("h", "qx", "qy", "w", "p"):
+            assert np.array_equal(sg[f], so[f]), (done, f, np.max(np.abs(sg[f] - so[f])))
+        ig, io = g.info(), o.info()
+        assert ig.iters_total == io.iters_total and ig.t == io.t and ig.clamps == io.clamps
+        wet = so["h"] > 1e-5
+        wet_max = max(wet_max, int(np.sum(wet & ~wet0)))
         probe.set_state(so["h"], so["qx"], so["qy"], so["w"], so["p"])
         b = probe.breaking(o.info().dt_last)
         broke = max(broke, int(np.sum(b["w"] != so["w"])))
+        # default solver (BiCGStab to 1e-12) against the same oracle run (Jacobi to 1e-6 increment): two
+        # different valid solves of every pressure system
+        assert np.mean((s0["h"] > 1e-5) != wet) <= 0.01, done
+        assert np.max(np.abs(s0["h"] - so["h"])) <= 0.05 * cfg["h0"], done
+        assert g0.info().t == pytest.approx(io.t, rel=1e-6)
     assert broke > 0          # the breaking criterion (9) was active inside a compared window
     assert wet_max > 8 * 100  # the shoreline ran up by more than 5 m of beach (100 cells per row)
     ig, io = g.info(), o.info()
-    # clamps: the bulk are round-off sized events at still dry cells (R24: their count is not unique
-    # across two valid solves); the thin film produces a few real ones, equal in number on both sides
-    assert list(ig.clamp_hist)[2:] == list(io.clamp_hist)[2:] and sum(list(io.clamp_hist)[2:]) > 0
-    assert ig.clamp_hist[0] > 0 and io.clamp_hist[0] > 0 and ig.clamp_max == pytest.approx(io.clamp_max, rel=1e-6)
+    assert list(ig.clamp_hist) == list(io.clamp_hist) and sum(list(io.clamp_hist)[2:]) > 0
+    assert ig.clamp_max == io.clamp_max
+    g0.close()
 
 
 def test_config4_checkpoint_restart_on_breaking_onset_and_maximum_runup(O, G):

@@ -1120,3 +1120,150 @@ def test_all_dry_domain_is_left_unchanged(O):
         assert i.dt_last == 0.0 and i.t == 0.0 and i.steps == 3 and i.iters_total == 0 and i.clamps == 0
         assert all(np.all(s[k] == 0.0) for k in ("h", "qx", "qy", "p"))
         assert np.array_equal(s["w"], st["w"])
+
+
+# ---------------------------------------------------------------- R30: w-advection variant of [7]
+# "(hw)_t + (hwu)_x = p ... matches with the one proposed in [7]"; with
+# h_t + q_x = 0 that is w_t + u w_x = p / h.  Reading R30: first-order upwind transport of
+# the node values with the 4-cell mean of the desingularised velocities.  Pinned against closed
+# forms of the transport equation, the maximum principle and the reduction to h w_t = p.
+def _advect_case(O, nx, ny, dx, dy, u, v, w, bcs=(OUT, OUT, OUT, OUT), h0=2.0):
+    H = np.full((ny, nx), h0)
+    o = O.Oracle(nx, ny, dx, dy, H, bc_xlo=bcs[0], bc_xhi=bcs[1], bc_ylo=bcs[2], bc_yhi=bcs[3],
+                 w_advect=1)
+    o.set_state(H, H * u, H * v, w, None)
+    return o
+
+
+def test_w_advection_linear_field_uniform_flow_is_exact(O):
+    # w = a x + b y under constant (u0, v0): w(t + dt) = w - dt (u0 a + v0 b) exactly (upwind
+    # differences of a linear field are exact), any sign of the velocities
+    nx, ny, dx, dy = 14, 11, 0.5, 0.25
+    X, Y = np.meshgrid(np.arange(nx + 1) * dx, np.arange(ny + 1) * dy)
+    a, b = 0.3, -1.1
+    w = a * X + b * Y
+    for u0, v0 in [(1.5, 0.7), (-1.5, 0.7), (1.5, -0.7), (-0.2, -2.0)]:
+        o = _advect_case(O, nx, ny, dx, dy, np.full((ny, nx), u0), np.full((ny, nx), v0), w)
+        wa = o.w_advect(0.05)
+        ref = w - 0.05 * (u0 * a + v0 * b)
+        assert np.max(np.abs(wa[1:-1, 1:-1] - ref[1:-1, 1:-1])) <= 1e-14      # away from the ghost maps
+
+
+@pytest.mark.parametrize("sgn", [1.0, -1.0])
+def test_w_advection_courant_one_shifts_by_one_node_upwind(O, sgn):
+    # u0 dt = dx: first-order upwind reproduces the exact solution w(x - u0 dt): a shift by one node
+    # in the direction of the flow (pins the upwind side and the sign of the transport term)
+    nx, ny, dx, dy = 24, 6, 0.4, 0.3
+    rng = np.random.default_rng(5)
+    w = np.repeat(rng.uniform(-1, 1, nx + 1)[None, :], ny + 1, axis=0)
+    w[:, -1] = w[:, 0]
+    u0 = 0.8 * sgn
+    o = _advect_case(O, nx, ny, dx, dy, np.full((ny, nx), u0), np.zeros((ny, nx)), w, bcs=(PER, PER, PER, PER))
+    wa = o.w_advect(dx / abs(u0))
+    ref = np.roll(w[:, :-1], 1 if sgn > 0 else -1, axis=1)
+    assert np.max(np.abs(wa[:, :-1] - ref)) <= 1e-15
+    # same in y
+    o = _advect_case(O, ny, nx, dy, dx, np.zeros((nx, ny)), np.full((nx, ny), u0), w.T.copy(), bcs=(PER, PER, PER, PER))
+    wa = o.w_advect(dx / abs(u0))
+    assert np.max(np.abs(wa[:-1, :] - ref.T)) <= 1e-15
+
+
+def test_w_advection_node_velocity_is_the_four_cell_mean_and_vanishes_at_a_wall(O):
+    # u = c x y at the cell centres: the mean over the four cells around node (X, Y) is exactly
+    # c X Y (a two-cell or diagonal average would be off by c dx dy / 4); w = a x  =>
+    # w* = w - dt (c X Y) a at interior nodes.  At an x-wall node the mirrored ghost cells carry -u:
+    # the normal node velocity is 0 and w there does not move.
+    nx, ny, dx, dy = 12, 10, 0.5, 0.4
+    xc, yc = np.meshgrid((np.arange(nx) + 0.5) * dx, (np.arange(ny) + 0.5) * dy)
+    X, Y = np.meshgrid(np.arange(nx + 1) * dx, np.arange(ny + 1) * dy)
+    c, a, dt = 0.37, 0.9, 0.02
+    w = a * X
+    o = _advect_case(O, nx, ny, dx, dy, c * xc * yc, np.zeros((ny, nx)), w, bcs=(WALL, WALL, OUT, OUT))
+    wa = o.w_advect(dt)
+    ref = w - dt * (c * X * Y) * a
+    assert np.max(np.abs(wa[1:-1, 1:-1] - ref[1:-1, 1:-1])) <= 1e-14
+    assert np.array_equal(wa[1:-1, 0], w[1:-1, 0]) and np.array_equal(wa[1:-1, -1], w[1:-1, -1])
+
+
+@pytest.mark.parametrize("bcs", [(PER, PER, PER, PER), (WALL, OUT, PER, PER), (OUT, OUT, WALL, WALL)])
+def test_w_advection_maximum_principle_under_the_cfl_time_step(O, bcs):
+    # with dt from (23) the update is a convex combination of a node and its upwind neighbours
+    st = inputs.random_smooth_state(30, 22, 0.3, 0.2, seed=12, depth=1.0, rough=0.4, dry_fraction=0.2)
+    o = O.Oracle(30, 22, 0.3, 0.2, st["H"], bc_xlo=bcs[0], bc_xhi=bcs[1], bc_ylo=bcs[2], bc_yhi=bcs[3],
+                 w_advect=1, cfl=1.0)
+    o.set_state(st["h"], 3.0 * st["qx"], 3.0 * st["qy"], st["w"])
+    wa = o.w_advect(o.compute_dt())
+    sl = (slice(0, -1 if bcs[2] == PER else None), slice(0, -1 if bcs[0] == PER else None))
+    assert wa[sl].max() <= st["w"][sl].max() + 1e-15 and wa[sl].min() >= st["w"][sl].min() - 1e-15
+    assert np.max(np.abs(wa - st["w"])) > 1e-3          # ... and it did transport something
+
+
+def test_w_advection_reduces_to_the_paper_scheme_when_the_fluid_is_at_rest(O):
+    # q = 0 in the stage input: the transport term vanishes identically, so one first-order stage of
+    # the variant is bit-identical to h w_t = p (L56, L104); with RK2 the second stage sees u != 0
+    # and the two models differ
+    st = inputs.random_smooth_state(26, 18, 0.3, 0.2, seed=21, depth=1.0, rough=0.3, dry_fraction=0.15)
+    z = np.zeros_like(st["h"])
+    res = {}
+    for adv in (0, 1):
+        for order in (1, 2):
+            o = O.Oracle(26, 18, 0.3, 0.2, st["H"], bc_xlo=WALL, bc_xhi=OUT, bc_ylo=PER, bc_yhi=PER,
+                         w_advect=adv, time_order=order)
+            o.set_state(st["h"], z, z, st["w"])
+            o.step(1)
+            res[adv, order] = o.get_state()
+    for k in ("h", "qx", "qy", "w", "p"):
+        assert np.array_equal(res[0, 1][k], res[1, 1][k]), k
+    assert np.max(np.abs(res[0, 2]["w"] - res[1, 2]["w"])) > 1e-9
+
+
+def test_w_advection_step_commutes_with_transposition_and_keeps_rest(O):
+    st = inputs.random_smooth_state(28, 20, 0.3, 0.2, seed=4, depth=1.0, rough=0.4, dry_fraction=0.15)
+    o1 = O.Oracle(28, 20, 0.3, 0.2, st["H"], bc_xlo=WALL, bc_xhi=OUT, bc_ylo=PER, bc_yhi=PER, w_advect=1)
+    o1.set_state(st["h"], st["qx"], st["qy"], st["w"])
+    o2 = O.Oracle(20, 28, 0.2, 0.3, st["H"].T.copy(), bc_xlo=PER, bc_xhi=PER, bc_ylo=WALL, bc_yhi=OUT, w_advect=1)
+    o2.set_state(st["h"].T.copy(), st["qy"].T.copy(), st["qx"].T.copy(), st["w"].T.copy())
+    o1.step(4), o2.step(4)
+    a, b = o1.get_state(), o2.get_state()
+    for k1, k2 in (("h", "h"), ("qx", "qy"), ("qy", "qx"), ("w", "w"), ("p", "p")):
+        np.testing.assert_allclose(a[k1], b[k2].T, rtol=0, atol=1e-10 * max(1.0, np.abs(a[k1]).max()))
+    # lake at rest over wet/dry bumps stays at rest with the variant on (P1)
+    cfg = inputs.make_config(2, nx=48, ny=40)
+    o = make(O, cfg, w_advect=1)
+    o.step(20)
+    s = o.get_state()
+    assert np.all(s["qx"] == 0.0) and np.all(s["qy"] == 0.0) and np.all(s["w"] == 0.0)
+
+
+def test_w_advection_total_energy_does_not_increase(O):
+    # L111: with the transport term "the system verifies an exact energy balance"; the discrete scheme
+    # (HLL diffusion, upwind transport) may only lose energy.  Closed flat periodic basin, Gaussian
+    # hump: E = sum[g eta^2 / 2 + h (u^2 + v^2) / 2] + sum_nodes[h_n w^2 / 2] is non-increasing and
+    # the variant stays close to the paper's h w_t = p ("no relevant differences", L113)
+    nx = ny = 48
+    dx = dy = 0.1
+    h0, g = 0.5, 9.81
+    xc, yc = np.meshgrid((np.arange(nx) + 0.5) * dx, (np.arange(ny) + 0.5) * dy)
+    eta0 = 0.05 * np.exp(-((xc - 2.4) ** 2 + (yc - 2.4) ** 2) / 0.3 ** 2)
+    H = np.full((ny, nx), h0)
+    z = np.zeros((ny, nx))
+
+    def energy(s):
+        h = s["h"]
+        e = np.sum(0.5 * g * (h - H) ** 2 + 0.5 * (s["qx"] ** 2 + s["qy"] ** 2) / h)
+        hn = 0.25 * (h + np.roll(h, 1, 0) + np.roll(h, 1, 1) + np.roll(np.roll(h, 1, 0), 1, 1))
+        return (e + np.sum(0.5 * hn * s["w"][:-1, :-1] ** 2)) * dx * dy
+
+    out = {}
+    for adv in (0, 1):
+        o = O.Oracle(nx, ny, dx, dy, H, bc_xlo=PER, bc_xhi=PER, bc_ylo=PER, bc_yhi=PER, w_advect=adv)
+        o.set_state(H + eta0, z, z)
+        E = [energy(o.get_state())]
+        for _ in range(30):
+            o.step(4)
+            E.append(energy(o.get_state()))
+        out[adv] = (np.array(E), o.get_state())
+    E1 = out[1][0]
+    assert np.all(np.diff(E1) <= 1e-12 * E1[0]) and E1[-1] > 0.5 * E1[0]
+    d = np.max(np.abs(out[1][1]["h"] - out[0][1]["h"]))
+    assert 0.0 < d < 0.02 * 0.05        # the two models differ, by little
