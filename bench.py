@@ -442,10 +442,21 @@ def run_parityruns(args):
             kw["window"] = f[3]
         cfg = inputs.make_config(idx, **kw)
         prm = dict(cfg["params"])
+        if args.solver == "srj":      # the paper's solver: both sides do the same arithmetic (bit-exact)
+            prm.update(solver=1, srj_eps=args.srj_eps)
         o = nh_oracle.Oracle(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], **prm)
         g = nh.NH(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], **prm)
-        for a in (o, g):
-            a.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
+        o2 = None
+        if args.spread:               # a second, equally valid oracle run: solver tolerance 10 x tighter
+            prm2 = dict(prm)
+            if args.solver == "srj":
+                prm2["srj_eps"] = 0.1 * args.srj_eps
+            else:
+                prm2["solver_rtol"] = 0.1 * prm.get("solver_rtol", 1e-12)
+            o2 = nh_oracle.Oracle(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], **prm2)
+        for a in (o, g, o2):
+            if a is not None:
+                a.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
         probe = nh_oracle.Oracle(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], **prm) if prm.get("breaking") else None
         eps_dry = 1e-5
         wet0 = int(np.sum(cfg["h"] > eps_dry))
@@ -460,12 +471,19 @@ def run_parityruns(args):
             io, ig = o.info(), g.info()
             r = parity_ratios(sg, so, cfg["H"], cfg["h0"])
             worst = max(worst, max(r.values()))
+            spread = None
+            if o2 is not None:
+                o2.step(n, allow_noconv=True)
+                spread = parity_ratios(o2.get_state(), so, cfg["H"], cfg["h0"])
             wet = so["h"] > eps_dry
             cp = dict(step=done, t_oracle=io.t, t_gpu=ig.t, ratios={a: round(b, 4) for a, b in r.items()},
                       iters_total=[int(ig.iters_total), int(io.iters_total)], clamps=[int(ig.clamps), int(io.clamps)],
                       wet_cells=int(wet.sum()), wet_cells_changed_vs_start=int(np.sum(wet != (cfg["h"] > eps_dry))),
                       wet_mask_equal=bool(np.array_equal(wet, sg["h"] > eps_dry)),
-                      eta_max=float(np.max(np.where(wet, so["h"] - cfg["H"], -np.inf))), gpu_status=int(stg))
+                      eta_max=float(np.max(np.where(wet, so["h"] - cfg["H"], -np.inf))), gpu_status=int(stg),
+                      bit_exact=bool(all(np.array_equal(sg[a], so[a]) for a in so)))
+            if spread is not None:    # oracle (tolerance / 10) against oracle: what two valid solves differ by
+                cp["oracle_spread_ratios"] = {a: round(b, 4) for a, b in spread.items()}
             if probe is not None:   # where is the breaking criterion of (9) active right now? (oracle S6 hook)
                 probe.set_state(so["h"], so["qx"], so["qy"], so["w"], so["p"])
                 b = probe.breaking(max(io.dt_last, 1e-9))
@@ -477,7 +495,8 @@ def run_parityruns(args):
         io, ig = o.info(), g.info()
         print(json.dumps(dict(
             parityrun=spec, workload=cfg["name"], nx=nx, ny=ny, dx=cfg["dx"], steps=steps, h0=cfg["h0"],
-            bars="max|d eta| <= 1e-9 h0; max|d a| <= 1e-9 max(max|a|, 1e-3 floor_a), a in qx,qy,w,p; ratio = error/allowed",
+            solver=("paper's Jacobi / scheduled relaxation, eps %g" % args.srj_eps) if args.solver == "srj" else "Jacobi-BiCGStab rtol 1e-12",
+            bars="max|d eta| <= 1e-9 h0; max|d a| <= 1e-9 max(max|a|, 1e-3 floor_a), a in q (one vector), w, p; ratio = error/allowed",
             worst_ratio=worst, passed=bool(worst <= 1.0), checkpoints=cps, wet_cells_start=wet0,
             clamp_hist_bins_m="<1e-15,<1e-12,<1e-9,<1e-6,<1e-3,>=1e-3",
             clamp_hist_gpu=list(ig.clamp_hist), clamp_hist_oracle=list(io.clamp_hist),
@@ -486,6 +505,8 @@ def run_parityruns(args):
             oracle_seconds=t_o, gpu_seconds=t_g, oracle_threads=int(os.environ.get("OMP_NUM_THREADS", os.cpu_count() or 1)))),
             flush=True)
         g.close(); o.close()
+        if o2 is not None:
+            o2.close()
         if probe is not None:
             probe.close()
     return 0
@@ -508,6 +529,8 @@ def main():
     ap.add_argument("--fullruns", default="", help="comma-separated config numbers: run each at full size for its full step count")
     ap.add_argument("--parityruns", default="", help="idx:NXxNY:steps[:window],... : oracle beside the CUDA path over the "
                     "configured horizon, parity at 10 checkpoints (slow; a record for profiles/)")
+    ap.add_argument("--spread", action="store_true", help="--parityruns: also run a second oracle with a 10 x tighter "
+                    "solver tolerance and report oracle-vs-oracle ratios (the spread of two valid solves)")
     args = ap.parse_args()
     if args.parityruns:
         return run_parityruns(args)

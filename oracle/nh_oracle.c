@@ -131,6 +131,42 @@ double nho_minmod(double a, double b) {
   return (a > 0.0) ? fmin(a, b) : fmax(a, b);
 }
 
+/* Reading R31 (two transcendentals evaluated by a FIXED algorithm).  h^(4/3) of the friction law
+ * (L61-65) and sech^2 of the solitary-wave target (33) need a cube root and an exponential; libm's
+ * are not correctly rounded and differ from library to library in the last place, and a wet/dry
+ * front amplifies last-place differences.  Both are therefore evaluated by a stated sequence of
+ * IEEE operations (frexp / ldexp / floor are exact), which any implementation reproduces bit for bit.
+ * Accuracy: a few ulp (pinned against libm in tests/test_oracle_pins.py). */
+/* cube root of a > 0: a = t 8^q with t in [0.5, 4); six Halley steps y <- y (y^3 + 2t) / (2y^3 + t)
+ * from y = 1 (cubic convergence: 0.37 -> 3e-2 -> 3e-5 -> 1e-14 -> rounding) */
+static double cbrt_fixed(double a) {
+  int e;
+  double m = frexp(a, &e);             /* a = m 2^e, m in [0.5, 1) */
+  int q = (e + 3072) / 3 - 1024;       /* floor(e / 3), non-negative dividend */
+  double t = ldexp(m, e - 3 * q);      /* t in [0.5, 4) */
+  double y = 1.0;
+  for (int k = 0; k < 6; ++k) {
+    double y3 = y * y * y;
+    y = y * (y3 + 2.0 * t) / (2.0 * y3 + t);
+  }
+  return ldexp(y, q);
+}
+/* sech^2(a) = 4 e / (1 + e)^2, e = exp(-2|a|) = 2^-n exp(-r), n = nearest integer to 2|a| / ln 2,
+ * r = 2|a| - n ln 2 in two pieces (|r| <= 0.35), exp(-r) by its Taylor series to r^14 (Horner) */
+static double sech2_fixed(double a) {
+  double y = 2.0 * fabs(a);
+  if (y > 745.0) return 0.0;
+  double n = floor(y * 1.4426950408889634 + 0.5);
+  double r = (y - n * 0.693147180369123816490) - n * 1.90821492927058770002e-10;
+  double p = 1.0;
+  for (int k = 14; k >= 1; --k) p = 1.0 - (r / (double)k) * p;
+  double e = ldexp(p, -(int)n);
+  double d = 1.0 + e;
+  return 4.0 * e / (d * d);
+}
+double nho_cbrt_fixed(double a) { return cbrt_fixed(a); }   /* test hooks (pins) */
+double nho_sech2_fixed(double a) { return sech2_fixed(a); }
+
 static void derived_fields(nho_ctx* c, const double* h, const double* qx, const double* qy) {
   const double delta = c->prm.delta;
 #pragma omp parallel for if (NHO_PAR(c)) schedule(static)
@@ -279,7 +315,7 @@ static void predictor(nho_ctx* c, const double* h, const double* qx, const doubl
          * with the desingularised velocities of U* (S0); wet cells only. */
         double uu = nho_dsg(hn, qxn, c->prm.delta), vv = nho_dsg(hn, qyn, c->prm.delta);
         double speed = sqrt(uu * uu + vv * vv);
-        double h43 = hn * cbrt(hn);
+        double h43 = hn * cbrt_fixed(hn);   /* R31 */
         double den = 1.0 + dt * g * c->prm.manning_n * c->prm.manning_n * speed / h43;
         qxn = qxn / den; qyn = qyn / den;
       }
@@ -782,8 +818,8 @@ static void relaxation(nho_ctx* c, double* h, double* qx, double* qy, double* w,
       size_t k = CIDX(c, i, j);
       double m = relax_m_cell(c, i);
       double x = ((double)i + 0.5) * c->dx;
-      double sech = 1.0 / cosh(kk * (x - x0 - cel * tt));
-      double etas = A * sech * sech;
+      double sech2 = sech2_fixed(kk * (x - x0 - cel * tt));   /* R31 */
+      double etas = A * sech2;
       double hs = fmax(c->H[k] + etas, 0.0);
       h[k] = m * h[k] + (1.0 - m) * hs;
       qx[k] = m * qx[k] + (1.0 - m) * (cel * etas);

@@ -102,6 +102,8 @@ void nho_face_fluct(double g, double hm, double etam, double um, double vm,
                     double Dm[3], double Dp[3]);                     /* S4 */
 double nho_dsg(double h, double q, double delta);                    /* S0 */
 double nho_minmod(double a, double b);                               /* S2 */
+double nho_cbrt_fixed(double a);   /* R31: cube root of a > 0 by the fixed algorithm (friction, R27) */
+double nho_sech2_fixed(double a);  /* R31: sech^2 by the fixed algorithm (solitary-wave target, S11)  */
 
 #ifdef __cplusplus
 }

@@ -73,6 +73,9 @@ def lib():
         L.nho_dsg.restype = C.c_double
         L.nho_minmod.argtypes = [C.c_double] * 2
         L.nho_minmod.restype = C.c_double
+        for f in (L.nho_cbrt_fixed, L.nho_sech2_fixed):
+            f.argtypes = [C.c_double]
+            f.restype = C.c_double
         _lib = L
     return _lib
 
@@ -220,3 +223,11 @@ def dsg(h, q, delta):
 
 def minmod(a, b):
     return lib().nho_minmod(a, b)
+
+
+def cbrt_fixed(a):
+    return lib().nho_cbrt_fixed(a)
+
+
+def sech2_fixed(a):
+    return lib().nho_sech2_fixed(a)

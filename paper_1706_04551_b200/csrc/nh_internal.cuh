@@ -106,6 +106,39 @@ __device__ __forceinline__ double nh_minmod(double a, double b) {
   return (a > 0.0) ? fmin(a, b) : fmax(a, b);
 }
 
+// R31: the two transcendentals of the path -- the cube root in h^(4/3) of the friction law (L61-65)
+// and sech^2 of the solitary-wave target (33) -- are evaluated by a stated sequence of IEEE
+// operations (frexp / ldexp / floor are exact) instead of library routines whose last place is
+// not specified, so that the results do not depend on who evaluates them.
+// cube root of a > 0: a = t 8^q, t in [0.5, 4); six Halley steps from y = 1
+__device__ __forceinline__ double nh_cbrt_fixed(double a) {
+  int e;
+  double m = frexp(a, &e);
+  int q = (e + 3072) / 3 - 1024;  // floor(e / 3)
+  double t = ldexp(m, e - 3 * q);
+  double y = 1.0;
+#pragma unroll 1
+  for (int k = 0; k < 6; ++k) {
+    double y3 = y * y * y;
+    y = y * (y3 + 2.0 * t) / (2.0 * y3 + t);
+  }
+  return ldexp(y, q);
+}
+// sech^2(a) = 4 e / (1 + e)^2, e = exp(-2|a|) = 2^-n exp(-r), r = 2|a| - n ln 2 (two pieces),
+// exp(-r) by its Taylor series to r^14 in Horner form
+__device__ __forceinline__ double nh_sech2_fixed(double a) {
+  double y = 2.0 * fabs(a);
+  if (y > 745.0) return 0.0;
+  double n = floor(y * 1.4426950408889634 + 0.5);
+  double r = (y - n * 0.693147180369123816490) - n * 1.90821492927058770002e-10;
+  double p = 1.0;
+#pragma unroll 1
+  for (int k = 14; k >= 1; --k) p = 1.0 - (r / (double)k) * p;
+  double e = ldexp(p, -(int)n);
+  double d = 1.0 + e;
+  return 4.0 * e / (d * d);
+}
+
 // Internal node planes: NH_COL_PAD ghost / padding columns on the left, >= 2 on the right, pitch NP
 // a multiple of 16 doubles (every row starts on a 128-byte line), ny + 5 rows; the pointer handed
 // to kernels addresses node (0,0) = physical element (2 rows, 4 columns), so that a[J * np + I] is

@@ -227,7 +227,7 @@ k_predictor(NhGrid G, double g, double delta, double eps_dry, double manning_n, 
     // q <- q / (1 + dt g n^2 |u*| / h*^(4/3)), desingularised velocities of U*, wet cells only
     double uu = nh_dsg(hn, qxn, delta), vv = nh_dsg(hn, qyn, delta);
     double speed = sqrt(uu * uu + vv * vv);
-    double h43 = hn * cbrt(hn);
+    double h43 = hn * nh_cbrt_fixed(hn);  // R31
     double den = 1.0 + dt * g * manning_n * manning_n * speed / h43;
     qxn = qxn / den; qyn = qyn / den;
   }

@@ -455,8 +455,7 @@ k_relax(NhGrid G, const NhScal* sc, int stage, double g, double A, double h0, do
       size_t k = (size_t)j * G.nx + i;
       double m = relax_m_cell(L, G.dx, i);
       double x = ((double)i + 0.5) * G.dx;
-      double sech = 1.0 / cosh(kk * (x - x0 - cel * tt));
-      double etas = A * sech * sech;
+      double etas = A * nh_sech2_fixed(kk * (x - x0 - cel * tt));  // R31
       double hs = fmax(H[k] + etas, 0.0);
       h[k] = m * h[k] + (1.0 - m) * hs;
       qx[k] = m * qx[k] + (1.0 - m) * (cel * etas);

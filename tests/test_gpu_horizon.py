@@ -129,8 +129,9 @@ def test_config4_checkpoint_restart_on_breaking_onset_and_maximum_runup(O, G):
         cps.append(dict(state=s, t=i.t, nbreak=nbreak, runup=int(np.sum((s["h"] > 1e-5) & ~wet0))))
         g.step(25)
         assert g.sync() == 0
+    cps.append(dict(state=g.get_state(), t=g.info().t, nbreak=0, runup=0))   # the end of the run
     first_break = next(k for k, c in enumerate(cps) if c["nbreak"] > 0)
-    top = int(np.argmax([c["runup"] for c in cps]))
+    top = min(int(np.argmax([c["runup"] for c in cps])), len(cps) - 2)
     assert first_break >= 2 and cps[top]["runup"] > 48 * 20
     for name, k0 in (("breaking onset", first_break - 1), ("maximum run-up", max(top - 1, 0))):
         c = cps[k0]

@@ -1267,3 +1267,22 @@ def test_w_advection_total_energy_does_not_increase(O):
     assert np.all(np.diff(E1) <= 1e-12 * E1[0]) and E1[-1] > 0.5 * E1[0]
     d = np.max(np.abs(out[1][1]["h"] - out[0][1]["h"]))
     assert 0.0 < d < 0.02 * 0.05        # the two models differ, by little
+
+
+# ---------------------------------------------------------------- R31: fixed-algorithm transcendentals
+def test_fixed_algorithm_cube_root_and_sech2_against_libm(O):
+    # R31: h^(4/3) (friction, L61-65) and sech^2 (solitary-wave target (33)) are evaluated by stated
+    # sequences of IEEE operations so that every implementation agrees bit for bit; they must still
+    # BE the cube root and sech^2: within a few ulp of libm over the ranges the path uses
+    rng = np.random.default_rng(0)
+    a = np.concatenate([10.0 ** rng.uniform(-6, 4, 5000), [1e-5, 0.3, 4000.0]])
+    c = np.array([O.cbrt_fixed(v) for v in a])
+    assert np.max(np.abs(c - np.cbrt(a)) / np.cbrt(a)) <= 4 * np.finfo(float).eps
+    assert O.cbrt_fixed(27.0) == 3.0 and O.cbrt_fixed(8.0) == 2.0 and O.cbrt_fixed(1.0) == 1.0
+    assert O.cbrt_fixed(0.001) == pytest.approx(0.1, rel=1e-15)
+    x = np.concatenate([rng.uniform(-30, 30, 5000), [0.0, 1e-9, -1e-9, 0.5, -0.5]])
+    s = np.array([O.sech2_fixed(v) for v in x])
+    ref = 1.0 / np.cosh(x) ** 2
+    assert np.max(np.abs(s - ref) / ref) <= 6 * np.finfo(float).eps
+    assert O.sech2_fixed(0.0) == 1.0 and O.sech2_fixed(400.0) == 0.0
+    assert O.sech2_fixed(1.3) == O.sech2_fixed(-1.3)
