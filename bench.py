@@ -208,6 +208,8 @@ def run_b200(args):
     prm = dict(cfg["params"])
     if args.solver == "srj":
         prm.update(solver=1, srj_eps=args.srj_eps)
+    if args.precision == 32:      # the optional fp32 variant: labelled, never the headline
+        prm.update(precision=32, solver_rtol=1e-4)
     sim = nh.NH(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], stream=stream, **prm)
     sim.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
 
@@ -242,19 +244,25 @@ def run_b200(args):
     peak, peak_src = _peaks()
     sol_ms, sol_n = prof["solver"]
     node_iters = (iters + solves) * float(nn)          # + the polish iteration of every solve
-    bytes_unit = BYTES_PER_NODE_ITER
+    bytes_unit = BYTES_PER_NODE_ITER * (0.5 if args.precision == 32 else 1.0)
     if args.solver == "srj":   # one Jacobi sweep: reads x, b', 4 coefficients, writes x'
-        bytes_unit = 56.0
+        bytes_unit = 56.0 * (0.5 if args.precision == 32 else 1.0)
         node_iters = (iters + solves) * float(nn)      # + the sweep that meets the stopping rule
     achieved = bytes_unit * node_iters / (sol_ms * 1e-3) / 1e9 if sol_ms > 0 else 0.0
-    traffic = None
+    # bytes this kernel itself must move per node-iteration: the matrix-free two-pass
+    # iteration reads / writes 18 planes (144 B in fp64) -- SURVEY 8(d)'s "lower bound"; k_srj: 7 planes.
+    kernel_unit = (56.0 if args.solver == "srj" else 144.0) * (0.5 if args.precision == 32 else 1.0)
+    # measured DRAM traffic: ncu dram__bytes_read + write per node-iteration of the SAME kernel
+    # (profiles/traffic.json names the capture), scaled by this run's node-iterations per launch
+    traffic, traffic_unit = None, None
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tp):
         try:
             tj = json.load(open(tp))
-            if tj.get("workload") == cfg["name"] and tj.get("nx") == nx and tj.get("ny") == ny \
-                    and args.solver == "bicgstab":
-                traffic = tj.get("dram_bytes_per_launch")
+            key = ("k_srj" if args.solver == "srj" else "k_bicgstab") + ("_f32" if args.precision == 32 else "_f64")
+            if key in tj.get("dram_bytes_per_node_iteration", {}) and nx * ny >= 4096 * 4096:
+                traffic_unit = float(tj["dram_bytes_per_node_iteration"][key])
+                traffic = traffic_unit * node_iters / max(sol_n, 1)
         except Exception:
             pass
     roofline = {
@@ -262,7 +270,13 @@ def run_b200(args):
                                   " (one cooperative launch per pressure solve)",
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
         "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0,
-        "bytes_per_node_iteration": bytes_unit, "launches": sol_n,
+        "bytes_per_node_iteration": bytes_unit, "bytes_source": "SURVEY.md 8(d) per-unit figure (fp32 variant: half)",
+        "kernel_bytes_per_node_iteration": kernel_unit,
+        "frac_of_kernel_bytes": (kernel_unit / bytes_unit) * achieved / peak,
+        "traffic_per_node_iteration": traffic_unit,
+        "traffic_note": "derived: ncu DRAM bytes per node-iteration of this kernel (profiles/traffic.json) x this run's "
+                        "node-iterations per launch" if traffic is not None else None,
+        "launches": sol_n,
         "avg_launch_ms": sol_ms / max(sol_n, 1),
         "iterations_per_launch": (iters + solves) / max(solves, 1),
         "phase_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
@@ -297,9 +311,10 @@ def run_b200(args):
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": f"configs[{args.config - 1}] {cfg['name']} {nx}x{ny} cells, dx={cfg['dx']} m",
-                   "solver": ("Jacobi-BiCGStab rtol 1e-12, device-resident convergence" if args.solver == "bicgstab"
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32" if args.precision == 32 else "f64", "data": "synthetic",
+        "config": {"workload": f"configs[{args.config - 1}] {cfg['name']} {nx}x{ny} cells, dx={cfg['dx']} m"
+                               + (" -- fp32 VARIANT (precision = 32, solver_rtol 1e-4), not the fp64 headline" if args.precision == 32 else ""),
+                   "solver": (("Jacobi-BiCGStab rtol %s, device-resident convergence" % ("1e-4" if args.precision == 32 else "1e-12")) if args.solver == "bicgstab"
                               else f"scheduled-relaxation Jacobi (paper's solver), increment rule (32) eps {args.srj_eps:g}"),
                    "iters_per_solve": iters / max(solves, 1), "time_order": 2,
                    "l2": "working set >> L2 (one fp64 plane = %.0f MB); no flush needed" % (8e-6 * nc)
@@ -320,6 +335,46 @@ def run_b200(args):
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
+    return 0
+
+
+def run_onesolve(args):
+    """One pressure solve in isolation, for the ncu capture behind profiles/traffic.json: W warm-up
+    steps, then nh_nonhydro_correct(dt_last) = exactly one launch of the solver kernel; prints its
+    iteration count so that DRAM bytes per node-iteration = ncu bytes / ((iterations + 1) x nodes).
+    Capture with: ncu --set full -k regex:k_bicgstab -s <2 W> -c 1 python bench.py --onesolve ..."""
+    import torch
+    from paper_1706_04551_b200 import inputs, nh
+    torch.cuda.set_device(0)
+    kw = {}
+    if args.nx:
+        kw["nx"] = args.nx
+    if args.ny:
+        kw["ny"] = args.ny
+    cfg = inputs.make_config(args.config, **kw)
+    prm = dict(cfg["params"])
+    if args.solver == "srj":
+        prm.update(solver=1, srj_eps=args.srj_eps)
+    if args.precision == 32:
+        prm.update(precision=32, solver_rtol=1e-4)
+    stream = torch.cuda.Stream()
+    sim = nh.NH(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["H"], stream=stream, **prm)
+    sim.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
+    sim.step(args.warmup)
+    sim.sync()
+    dt = sim.info().dt_last
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sim.profile(True)
+    e0.record(stream)
+    sim.nonhydro_correct(dt)
+    e1.record(stream)
+    st = sim.sync()
+    prof = sim.profile_read()
+    i = sim.info()
+    nn = (cfg["nx"] + 1) * (cfg["ny"] + 1)
+    print(json.dumps(dict(onesolve=cfg["name"], nx=cfg["nx"], ny=cfg["ny"], precision=args.precision, solver=args.solver,
+                          iterations=int(i.iters_last), node_iterations=(int(i.iters_last) + 1) * nn,
+                          solver_ms=prof["solver"][0], status=int(st), res_last=i.res_last)))
     return 0
 
 
@@ -444,6 +499,9 @@ def run_parityruns(args):
         prm = dict(cfg["params"])
         if args.solver == "srj":      # the paper's solver: both sides do the same arithmetic (bit-exact)
             prm.update(solver=1, srj_eps=args.srj_eps)
+        for kv in args.param:         # e.g. --param manning_n=0.01
+            k_, v_ = kv.split("=")
+            prm[k_] = float(v_) if "." in v_ or "e" in v_.lower() else int(v_)
         o = nh_oracle.Oracle(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], **prm)
         g = nh.NH(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], **prm)
         o2 = None
@@ -522,6 +580,8 @@ def main():
     ap.add_argument("--nx", type=int, default=0)
     ap.add_argument("--ny", type=int, default=0)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--precision", type=int, default=64, choices=[64, 32],
+                    help="32: the optional fp32 variant (labelled as such; the fp64 line is the headline)")
     ap.add_argument("--solver", default="bicgstab", choices=["bicgstab", "srj"],
                     help="bicgstab: north_star solver (default); srj: the paper's scheduled-relaxation Jacobi")
     ap.add_argument("--srj-eps", type=float, default=1e-5, help="stopping tolerance of eq. (32) for --solver srj")
@@ -529,9 +589,13 @@ def main():
     ap.add_argument("--fullruns", default="", help="comma-separated config numbers: run each at full size for its full step count")
     ap.add_argument("--parityruns", default="", help="idx:NXxNY:steps[:window],... : oracle beside the CUDA path over the "
                     "configured horizon, parity at 10 checkpoints (slow; a record for profiles/)")
+    ap.add_argument("--onesolve", action="store_true", help="one isolated pressure solve after --warmup steps (ncu capture)")
+    ap.add_argument("--param", action="append", default=[], help="--parityruns: override a parameter, key=value (repeatable)")
     ap.add_argument("--spread", action="store_true", help="--parityruns: also run a second oracle with a 10 x tighter "
                     "solver tolerance and report oracle-vs-oracle ratios (the spread of two valid solves)")
     args = ap.parse_args()
+    if args.onesolve:
+        return run_onesolve(args)
     if args.parityruns:
         return run_parityruns(args)
     if args.fullruns:

@@ -1,7 +1,7 @@
 /* nh_b200.h -- C ABI of libnh_b200.so: the per-time-step hot path of the hybrid finite-volume /
  * finite-difference projection scheme of Escalante, Morales de Luna & Castro (arXiv 1706.04551,
  * cited below as PAPER.md L<line>) for Yamazaki's depth-integrated non-hydrostatic system,
- * hand-written CUDA for NVIDIA B200 (sm_100a), fp64, SoA.
+ * hand-written CUDA for NVIDIA B200 (sm_100a), SoA, fp64 (optional fp32 variant: nh_params.precision).
  *
  * Every step of the path runs in CUDA kernels of this library; there is no CPU fallback.  No
  * torch types appear here: plain pointers and sizes.
@@ -72,7 +72,12 @@ typedef struct {
   int bc_xlo, bc_xhi, bc_ylo, bc_yhi; /* nh_bc; periodic must be set on both sides of a direction */
   int solver_maxit;   /* default 10000                                                      */
   int gen_on;         /* 1: generating relaxation zone active                               */
-  int precision;      /* 64 (fp64).  32 is not built yet: NH_EINVAL                         */
+  int precision;      /* 64 (default): fp64 throughout, the parity contract.  32: the optional fp32
+                         variant -- every field plane and its arithmetic in fp32 (eta = h - H is
+                         stored beside h so that metres of signal survive on kilometres of depth),
+                         dt, the clock and all dot products in fp64; arrays at this boundary stay
+                         fp64 (converted at set / get); solver_rtol below 1e-4 is raised to 1e-4.
+                         Tolerances against the fp64 oracle: DESIGN.md section 10                 */
   int solver;         /* 0 (default): Jacobi-preconditioned BiCGStab to solver_rtol (R14);
                          1: the paper's Jacobi method with scheduled relaxation and stopping
                          rule (32) (L507-514; R28): no dot products, results bit-identical

@@ -14,10 +14,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libnh_b200.so")
-SOURCES = ["nh_api.cu", "nh_predictor.cu", "nh_pressure.cu", "nh_solver.cu"]
+KERNEL_SOURCES = ["nh_core.cu", "nh_predictor.cu", "nh_pressure.cu", "nh_solver.cu"]  # once per precision
+ABI_SOURCE = "nh_abi.cu"
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-              "-fmad=false", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-shared",
-              "-cudart", "shared"]
+              "-fmad=false", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-cudart", "shared"]
+OBJ = os.path.join(HERE, "build")
 
 
 def _nvcc():
@@ -35,14 +36,36 @@ def _deps():
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Every kernel file and nh_core.cu are compiled twice (-DNH_PREC=64: namespace nh64, the fp64
+    contract; -DNH_PREC=32: namespace nh32, the fp32 variant), nh_abi.cu once; the objects are
+    compiled in parallel and linked into one shared library."""
     if not force and os.path.exists(LIB):
         m = os.path.getmtime(LIB)
         if all(m >= os.path.getmtime(p) for p in _deps()):
             return LIB
+    os.makedirs(OBJ, exist_ok=True)
     extra = os.environ.get("NH_NVCC_EXTRA", "").split()   # developer knob: extra -D switches for experiments
-    cmd = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
-        ["-I", INC, "-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
-    subprocess.run(cmd, check=True, cwd=HERE)
+    common = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-I", INC, "-c"]
+    jobs = []
+    for prec in (64, 32):
+        for src in KERNEL_SOURCES:
+            obj = os.path.join(OBJ, f"{os.path.splitext(src)[0]}_{prec}.o")
+            jobs.append((obj, common + [f"-DNH_PREC={prec}", "-o", obj, os.path.join(CSRC, src)]))
+    obj = os.path.join(OBJ, "nh_abi.o")
+    jobs.append((obj, common + ["-o", obj, os.path.join(CSRC, ABI_SOURCE)]))
+    procs = [(o, subprocess.Popen(cmd, cwd=HERE, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True))
+             for o, cmd in jobs]
+    failed = []
+    for o, pr in procs:
+        out, _ = pr.communicate()
+        if verbose or pr.returncode != 0:
+            sys.stderr.write(f"--- {os.path.basename(o)}\n{out}")
+        if pr.returncode != 0:
+            failed.append(o)
+    if failed:
+        raise subprocess.CalledProcessError(1, "nvcc -c", output=", ".join(failed))
+    subprocess.run([_nvcc(), "-shared", "-cudart", "shared", "-gencode", "arch=compute_100a,code=sm_100a",
+                    "-o", LIB] + [o for o, _ in jobs], check=True, cwd=HERE)
     return LIB
 
 

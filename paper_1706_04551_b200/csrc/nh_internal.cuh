@@ -9,6 +9,13 @@
 // correction therefore take every discrete decision (minmod branch, wet/dry test, emerging-bottom
 // clip, breaking flag, clamp) on the same values a plain CPU evaluation of the paper's formulas
 // sees; only the Krylov solver's dot products are summed in a different (tree) order.
+//
+// Precision.  Every kernel file and nh_core.cu are compiled twice, with NH_PREC = 64 (namespace
+// nh64, real = double: the contract above) and NH_PREC = 32 (namespace nh32, real = float: the
+// optional fp32 variant of north_star -- all field planes and their arithmetic in fp32, eta stored
+// beside h so that metres of signal survive on kilometres of depth, the scalar reductions (dt, dot
+// products, the clock) in fp64).  RC(x) types a literal as real.  nh_abi.cu
+// holds the extern "C" entry points and dispatches on nh_params.precision.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -18,13 +25,25 @@
 
 #include "../../include/nh_b200.h"
 
-struct NhGrid {
-  int nx, ny;    // cells
-  int nnx, nny;  // distinct node lines: n in a periodic direction, n+1 otherwise
-  int np;        // internal node pitch (nh_node_pitch: multiple of 16, ghost / padding columns on both sides)
-  int bxlo, bxhi, bylo, byhi;
-  double dx, dy;
-};
+#ifndef NH_PREC
+#define NH_PREC 64
+#endif
+#if NH_PREC == 64
+#define NH_NS nh64
+#define NH_REAL double
+#define NH_REAL2 double2
+#elif NH_PREC == 32
+#define NH_NS nh32
+#define NH_REAL float
+#define NH_REAL2 float2
+#else
+#error "NH_PREC must be 64 or 32"
+#endif
+#define RC(x) ((NH_REAL)(x))
+
+#ifndef NH_SHARED_TYPES
+#define NH_SHARED_TYPES
+
 
 // Device-resident scalars: the time step, the clock and the counters never visit the host
 // inside nh_step.
@@ -47,20 +66,37 @@ struct NhScal {
 };
 
 enum { NH_FLAG_NOCONV = 1, NH_FLAG_NAN = 2, NH_FLAG_BADSTATE = 4 };
+#endif  // NH_SHARED_TYPES
+
+namespace NH_NS {
+
+typedef NH_REAL real;
+typedef NH_REAL2 real2;
+// grid geometry handed to every kernel by value
+struct NhGrid {
+  int nx, ny;    // cells
+  int nnx, nny;  // distinct node lines: n in a periodic direction, n+1 otherwise
+  int np;        // internal node pitch (nh_node_pitch: multiple of 16, ghost / padding columns on both sides)
+  int bxlo, bxhi, bylo, byhi;
+  real dx, dy;
+};
+
+constexpr bool kEta = (NH_PREC == 32);  // eta stored beside h (fp32 variant)
+__host__ __device__ __forceinline__ real2 make_real2(real a, real b) { real2 v; v.x = a; v.y = b; return v; }
 
 // ---- S1: ghost access by index maps (R9) ------------------------------------------------
 // cells: periodic wraps; wall / outflow mirror (-1->0, -2->1, n->n-1, n+1->n-2); sgn = -1 only
 // in a wall ghost (applied by the caller to the normal discharge / velocity).
-__device__ __forceinline__ int nh_map_cell(int i, int n, int bclo, int bchi, double& sgn) {
-  sgn = 1.0;
+__device__ __forceinline__ int nh_map_cell(int i, int n, int bclo, int bchi, real& sgn) {
+  sgn = RC(1.0);
   if (i < 0) {
     if (bclo == NH_BC_PERIODIC) return i + n;
-    if (bclo == NH_BC_WALL) sgn = -1.0;
+    if (bclo == NH_BC_WALL) sgn = -RC(1.0);
     return -1 - i;
   }
   if (i >= n) {
     if (bchi == NH_BC_PERIODIC) return i - n;
-    if (bchi == NH_BC_WALL) sgn = -1.0;
+    if (bchi == NH_BC_WALL) sgn = -RC(1.0);
     return 2 * n - 1 - i;
   }
   return i;
@@ -84,26 +120,26 @@ __device__ __forceinline__ int nh_map_node(int I, int n, int bclo) {
 }
 
 // S0: desingularised velocity u = sqrt(2) h q / sqrt(h^4 + max(h^4, delta^4))  (L447-451)
-#define NH_SQRT2 1.4142135623730951
-__device__ __forceinline__ double nh_dsg(double h, double q, double delta) {
-  double h2 = h * h, h4 = h2 * h2;
-  double d2 = delta * delta, d4 = d2 * d2;
-  double den = sqrt(h4 + fmax(h4, d4));
-  double num = NH_SQRT2 * h * q;
+#define NH_SQRT2 RC(1.4142135623730951)
+__device__ __forceinline__ real nh_dsg(real h, real q, real delta) {
+  real h2 = h * h, h4 = h2 * h2;
+  real d2 = delta * delta, d4 = d2 * d2;
+  real den = sqrt(h4 + fmax(h4, d4));
+  real num = NH_SQRT2 * h * q;
   // 0 / den = 0 (den > 0): same bits, but a zero dividend would send the fp64 division down its slow
   // path, and still water is common (2.8 M of 3.5 M warp-divisions on the config-5 basin)
-  return (num == 0.0) ? num : num / den;
+  return (num == RC(0.0)) ? num : num / den;
 }
 // R16: dinv(h) = sqrt(2) h / sqrt(h^4 + max(h^4, delta^4))  (= 1/h for h >= delta)
-__device__ __forceinline__ double nh_dinv_h(double h, double delta) {
-  double h2 = h * h, h4 = h2 * h2;
-  double d2 = delta * delta, d4 = d2 * d2;
+__device__ __forceinline__ real nh_dinv_h(real h, real delta) {
+  real h2 = h * h, h4 = h2 * h2;
+  real d2 = delta * delta, d4 = d2 * d2;
   return (NH_SQRT2 * h) / sqrt(h4 + fmax(h4, d4));
 }
 // S2: minmod(a,b) = 0 if ab <= 0 else sign(a) min(|a|,|b|)  (L335)
-__device__ __forceinline__ double nh_minmod(double a, double b) {
-  if (a * b <= 0.0) return 0.0;
-  return (a > 0.0) ? fmin(a, b) : fmax(a, b);
+__device__ __forceinline__ real nh_minmod(real a, real b) {
+  if (a * b <= RC(0.0)) return RC(0.0);
+  return (a > RC(0.0)) ? fmin(a, b) : fmax(a, b);
 }
 
 // R31: the two transcendentals of the path -- the cube root in h^(4/3) of the friction law (L61-65)
@@ -111,32 +147,32 @@ __device__ __forceinline__ double nh_minmod(double a, double b) {
 // operations (frexp / ldexp / floor are exact) instead of library routines whose last place is
 // not specified, so that the results do not depend on who evaluates them.
 // cube root of a > 0: a = t 8^q, t in [0.5, 4); six Halley steps from y = 1
-__device__ __forceinline__ double nh_cbrt_fixed(double a) {
+__device__ __forceinline__ real nh_cbrt_fixed(real a) {
   int e;
-  double m = frexp(a, &e);
+  real m = frexp(a, &e);
   int q = (e + 3072) / 3 - 1024;  // floor(e / 3)
-  double t = ldexp(m, e - 3 * q);
-  double y = 1.0;
+  real t = ldexp(m, e - 3 * q);
+  real y = RC(1.0);
 #pragma unroll 1
   for (int k = 0; k < 6; ++k) {
-    double y3 = y * y * y;
-    y = y * (y3 + 2.0 * t) / (2.0 * y3 + t);
+    real y3 = y * y * y;
+    y = y * (y3 + RC(2.0) * t) / (RC(2.0) * y3 + t);
   }
   return ldexp(y, q);
 }
 // sech^2(a) = 4 e / (1 + e)^2, e = exp(-2|a|) = 2^-n exp(-r), r = 2|a| - n ln 2 (two pieces),
 // exp(-r) by its Taylor series to r^14 in Horner form
-__device__ __forceinline__ double nh_sech2_fixed(double a) {
-  double y = 2.0 * fabs(a);
-  if (y > 745.0) return 0.0;
-  double n = floor(y * 1.4426950408889634 + 0.5);
-  double r = (y - n * 0.693147180369123816490) - n * 1.90821492927058770002e-10;
-  double p = 1.0;
+__device__ __forceinline__ real nh_sech2_fixed(real a) {
+  real y = RC(2.0) * fabs(a);
+  if (y > RC(745.0)) return RC(0.0);
+  real n = floor(y * RC(1.4426950408889634) + RC(0.5));
+  real r = (y - n * RC(0.693147180369123816490)) - n * RC(1.90821492927058770002e-10);
+  real p = RC(1.0);
 #pragma unroll 1
-  for (int k = 14; k >= 1; --k) p = 1.0 - (r / (double)k) * p;
-  double e = ldexp(p, -(int)n);
-  double d = 1.0 + e;
-  return 4.0 * e / (d * d);
+  for (int k = 14; k >= 1; --k) p = RC(1.0) - (r / (real)k) * p;
+  real e = ldexp(p, -(int)n);
+  real d = RC(1.0) + e;
+  return RC(4.0) * e / (d * d);
 }
 
 // Internal node planes: NH_COL_PAD ghost / padding columns on the left, >= 2 on the right, pitch NP
@@ -153,7 +189,7 @@ inline int nh_node_pitch(int nnx) {
 }
 
 // ---- context ------------------------------------------------------------------------------
-struct nh_ctx {
+struct Ctx {
   NhGrid g;
   nh_params prm;
   cudaStream_t stream;
@@ -166,22 +202,25 @@ struct nh_ctx {
 
   size_t nc, nn;  // cells, nodes (public node layout)
   // cells
-  double* H;
-  double *h[3], *qx[3], *qy[3];  // three state slots (rotating): current, stage 1, stage 2
-  double *qx1, *qy1;             // predictor output q*
-  double *qx2, *qy2;             // q** (breaking on)
-  double* z;                     // z = 2 eta - h of U*
-  double *hc, *zc;               // h, z of U* in the node layout shifted by one column, ghost cells
+  real* H;
+  real* eta[3];   // fp32 variant only (kEta): eta = h - H of the three state slots, the master copy
+  double* Hd;     // fp32 variant only: the bathymetry as given (fp64), for eta = h - H at set / get
+  double* stage;  // fp32 variant only: fp64 staging plane for set / get (max(cells, nodes) doubles)
+  real *h[3], *qx[3], *qy[3];  // three state slots (rotating): current, stage 1, stage 2
+  real *qx1, *qy1;             // predictor output q*
+  real *qx2, *qy2;             // q** (breaking on)
+  real* z;                     // z = 2 eta - h of U*
+  real *hc, *zc;               // h, z of U* in the node layout shifted by one column, ghost cells
                                  // filled (operands of the matrix-free solver, nh_solver.cu)
   unsigned char *flag_c, *flag_n;
   // nodes
-  double* w[3];
-  double* w2;  // w** (breaking on)
-  double* wadv;  // w after the transport step of the w-advection variant (R30)
-  double* p;   // pressure multiplier p~ (warm start of the next solve)
-  double* b;   // right-hand side
-  double *dg, *dinv, *cE, *cW, *cN, *cS;  // diag(A), its inverse, column-scaled off-diagonals
-  double *ky, *kr, *krB, *kr0, *kpA, *kpB, *kvA, *kvB, *kt;  // BiCGStab vectors (r, p, v double-buffered)
+  real* w[3];
+  real* w2;  // w** (breaking on)
+  real* wadv;  // w after the transport step of the w-advection variant (R30)
+  real* p;   // pressure multiplier p~ (warm start of the next solve)
+  real* b;   // right-hand side
+  real *dg, *dinv, *cE, *cW, *cN, *cS;  // diag(A), its inverse, column-scaled off-diagonals
+  real *ky, *kr, *krB, *kr0, *kpA, *kpB, *kvA, *kvB, *kt;  // BiCGStab vectors (r, p, v double-buffered)
   double* pub;   // dense (nx+1) x (ny+1) staging plane for the public node layout
   std::vector<void*> raw;  // allocation bases (node planes are handed out offset to node (0,0))
   double* part;  // per-CTA partial sums of the solver
@@ -198,40 +237,48 @@ struct nh_ctx {
   std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_ev[NH_PROF_CATS];
 };
 
+// fp32 variant: the eta plane that goes with a state slot's h plane (nullptr in the fp64 build)
+inline real* nh_eta_of(const Ctx* c, const real* h) {
+  if (kEta)
+    for (int s = 0; s < 3; ++s)
+      if (c->h[s] == h) return c->eta[s];
+  return nullptr;
+}
+
 // ---- kernel launchers (each enqueues on c->stream and bumps c->launches) --------------------
 // nh_predictor.cu
-void nh_launch_lambda(nh_ctx* c, const double* h, const double* qx, const double* qy);
-void nh_launch_set_dt(nh_ctx* c, double dt_fixed /* <=0: CFL from lam */);
-void nh_launch_end_step(nh_ctx* c, int advance_time);
-void nh_launch_predictor(nh_ctx* c, const double* h, const double* qx, const double* qy,
-                         double* h1, double* qx1, double* qy1);
-void nh_launch_combine(nh_ctx* c, double* h0, double* qx0, double* qy0, double* w0,
-                       const double* h2, const double* qx2, const double* qy2, const double* w2);
-void nh_launch_validate(nh_ctx* c, const double* h, const double* qx, const double* qy);
+void nh_launch_lambda(Ctx* c, const real* h, const real* qx, const real* qy);
+void nh_launch_set_dt(Ctx* c, double dt_fixed /* <=0: CFL from lam */);
+void nh_launch_end_step(Ctx* c, int advance_time);
+void nh_launch_predictor(Ctx* c, const real* h, const real* qx, const real* qy,
+                         real* h1, real* qx1, real* qy1);
+void nh_launch_combine(Ctx* c, real* h0, real* qx0, real* qy0, real* w0,
+                       const real* h2, const real* qx2, const real* qy2, const real* w2);
+void nh_launch_validate(Ctx* c, const real* h, const real* qx, const real* qy);
 // nh_pressure.cu
-void nh_launch_compute_z(nh_ctx* c, const double* h, double* z);
-void nh_launch_cell_planes(nh_ctx* c, const double* h);  // z (dense) and hc, zc (solver 0)
-void nh_launch_breaking(nh_ctx* c, const double* h, const double* qx1, const double* qy1,
-                        const double* w_in, double* qx2, double* qy2, double* w2);
-void nh_launch_rhs(nh_ctx* c, const double* h, const double* qx, const double* qy, const double* z,
-                   const double* w, double* b, int constraint_only);
-void nh_launch_coeffs(nh_ctx* c, const double* h, const double* z);  // -> dg, dinv, raw cE..cS
-void nh_launch_scale_coeffs(nh_ctx* c);  // solver 0: cX *= dinv(neighbour)
-void nh_launch_scale_rows(nh_ctx* c, const double* b, double* bp);
-void nh_launch_assemble_rows(nh_ctx* c, const double* h, const double* qx, const double* qy,
-                             const double* z, const double* w, double* bp);  // solver 1: rhs + rows + scaling fused  // solver 1: cX *= dinv, bp = b dinv, rho, max|bp|
-void nh_launch_apply_A(nh_ctx* c, const double* h, const double* z, const double* x, double* y);
-void nh_launch_correct(nh_ctx* c, const double* h, const double* z, const double* qx2,
-                       const double* qy2, const double* w2, const double* p, double* qx_out,
-                       double* qy_out, double* w_out);
-void nh_launch_w_advect(nh_ctx* c, const double* h, const double* qx, const double* qy,
-                        const double* w_in, double* w_out);  // R30
-void nh_launch_relax(nh_ctx* c, double* h, double* qx, double* qy, double* w, double* p, int stage);
-void nh_launch_absorb(nh_ctx* c, double* h, double* qx, double* qy, double* w, double* p);
-void nh_launch_nodes_out(nh_ctx* c, const double* src, double* dst);
+void nh_launch_compute_z(Ctx* c, const real* h, real* z);
+void nh_launch_cell_planes(Ctx* c, const real* h);  // z (dense) and hc, zc (solver 0)
+void nh_launch_breaking(Ctx* c, const real* h, const real* qx1, const real* qy1,
+                        const real* w_in, real* qx2, real* qy2, real* w2);
+void nh_launch_rhs(Ctx* c, const real* h, const real* qx, const real* qy, const real* z,
+                   const real* w, real* b, int constraint_only);
+void nh_launch_coeffs(Ctx* c, const real* h, const real* z);  // -> dg, dinv, raw cE..cS
+void nh_launch_scale_coeffs(Ctx* c);  // solver 0: cX *= dinv(neighbour)
+void nh_launch_scale_rows(Ctx* c, const real* b, real* bp);
+void nh_launch_assemble_rows(Ctx* c, const real* h, const real* qx, const real* qy,
+                             const real* z, const real* w, real* bp);  // solver 1: rhs + rows + scaling fused  // solver 1: cX *= dinv, bp = b dinv, rho, max|bp|
+void nh_launch_apply_A(Ctx* c, const real* h, const real* z, const real* x, real* y);
+void nh_launch_correct(Ctx* c, const real* h, const real* z, const real* qx2,
+                       const real* qy2, const real* w2, const real* p, real* qx_out,
+                       real* qy_out, real* w_out);
+void nh_launch_w_advect(Ctx* c, const real* h, const real* qx, const real* qy,
+                        const real* w_in, real* w_out);  // R30
+void nh_launch_relax(Ctx* c, real* h, real* qx, real* qy, real* w, real* p, int stage);
+void nh_launch_absorb(Ctx* c, real* h, real* qx, real* qy, real* w, real* p);
+void nh_launch_nodes_out(Ctx* c, const real* src, double* dst);
 // nh_solver.cu
-int nh_solver_setup(nh_ctx* c);  // occupancy -> cooperative grid, partial buffer
-void nh_launch_solve(nh_ctx* c, const double* b, double* x, int count_stats);
+int nh_solver_setup(Ctx* c);  // occupancy -> cooperative grid, partial buffer
+void nh_launch_solve(Ctx* c, const real* b, real* x, int count_stats);
 
 #define NH_CUDA_OK(c, call)                                                                   \
   do {                                                                                        \
@@ -242,3 +289,5 @@ void nh_launch_solve(nh_ctx* c, const double* b, double* x, int count_stats);
       (c)->host_status = NH_ECUDA;                                                            \
     }                                                                                         \
   } while (0)
+
+}  // namespace NH_NS

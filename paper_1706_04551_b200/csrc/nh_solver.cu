@@ -52,7 +52,10 @@
 
 namespace cg = cooperative_groups;
 
+namespace NH_NS {
 namespace {
+
+#define D(x) ((double)(x))  // dot products, norms and the scalars of the method are fp64 in both builds
 
 #ifndef NH_NT
 #define NH_NT 192
@@ -72,15 +75,15 @@ constexpr int MAXDOT = 5;
 struct SolveP {
   NhGrid G;
   int nstrips, R, nbands;  // strips of SW columns, band height, bands
-  const double *hc, *zc;   // cell planes h, z = 2 eta - h of U* (node layout shifted by one column)
-  const double* b;
-  double* x;               // the iterate: start vector in, solution out (the pressure plane)
-  double *r0, *t;          // shadow residual (unscaled); t^
-  double *rA, *rB, *pA, *pB, *vA, *vB;  // r^, p^, v^ (double-buffered)
+  const real *hc, *zc;   // cell planes h, z = 2 eta - h of U* (node layout shifted by one column)
+  const real* b;
+  real* x;               // the iterate: start vector in, solution out (the pressure plane)
+  real *r0, *t;          // shadow residual (unscaled); t^
+  real *rA, *rB, *pA, *pB, *vA, *vB;  // r^, p^, v^ (double-buffered)
   double* part;  // [2][MAXDOT][gridDim.x]
   NhScal* sc;
   double rtol;
-  double miex, miey;  // -1 / (8 dx^2), -1 / (8 dy^2)
+  real miex, miey;  // -1 / (8 dx^2), -1 / (8 dy^2)
   int maxit;
   int count_stats;
 };
@@ -104,7 +107,7 @@ __device__ __forceinline__ int ghost_image(int I, int n, int bclo) {
 }
 
 // store a real node value and its ghost images (slow path: boundary nodes only)
-__device__ __forceinline__ void store_images(const NhGrid& G, double* a, int I, int J, double v) {
+__device__ __forceinline__ void store_images(const NhGrid& G, real* a, int I, int J, real v) {
   int gi = ghost_image(I, G.nnx, G.bxlo), gj = ghost_image(J, G.nny, G.bylo);
   a[nidx(G, I, J)] = v;
   if (gi != -2) a[nidx(G, gi, J)] = v;
@@ -178,20 +181,20 @@ __device__ __forceinline__ Unit make_unit(const SolveP& P, int u, int lane) {
 }
 
 // 16-byte load of the lane's column pair of row j
-__device__ __forceinline__ double2 ld2(const double* a, const NhGrid& G, int c0, int j) {
-  return *reinterpret_cast<const double2*>(a + nidx(G, c0, j));
+__device__ __forceinline__ real2 ld2(const real* a, const NhGrid& G, int c0, int j) {
+  return *reinterpret_cast<const real2*>(a + nidx(G, c0, j));
 }
 
 // store the lane's pair of row j (owned columns only) and its ghost images: the same pair again on
 // the ghost row of a boundary row, single values on the ghost column of a boundary column (the
 // warps of the first and last strip used to take a scalar path for every row and finished 8 %
 // (8192^2) to 34 % (2048^2) after the others, which every pass then waited for)
-__device__ __forceinline__ void st2(double* a, const SolveP& P, const Unit& U, int j, double2 v) {
+__device__ __forceinline__ void st2(real* a, const SolveP& P, const Unit& U, int j, real2 v) {
   const NhGrid& G = P.G;
   const int gj = ghost_image(j, G.nny, G.bylo);
   if (U.own1) {  // own1 implies own0
-    *reinterpret_cast<double2*>(a + nidx(G, U.c0, j)) = v;
-    if (gj != -2) *reinterpret_cast<double2*>(a + nidx(G, U.c0, gj)) = v;
+    *reinterpret_cast<real2*>(a + nidx(G, U.c0, j)) = v;
+    if (gj != -2) *reinterpret_cast<real2*>(a + nidx(G, U.c0, gj)) = v;
   } else if (U.own0) {
     a[nidx(G, U.c0, j)] = v.x;
     if (gj != -2) a[nidx(G, U.c0, gj)] = v.x;
@@ -210,56 +213,56 @@ __device__ __forceinline__ void st2(double* a, const SolveP& P, const Unit& U, i
 // of h and one of z are loaded, 16 bytes per node instead of the 32 of four stored coefficients.
 #define NH_FULL 0xffffffffu
 struct Coef {  // row of A at the lane's two nodes: A_E, A_W, A_N, A_S, A_C (S8)
-  double e[2], w[2], n[2], s[2], c[2];
+  real e[2], w[2], n[2], s[2], c[2];
 };
-__device__ __forceinline__ void lane3(double2 own, double (&q)[3]) {
+__device__ __forceinline__ void lane3(real2 own, real (&q)[3]) {
   q[0] = own.x; q[1] = own.y; q[2] = __shfl_down_sync(NH_FULL, own.x, 1);
 }
 struct March {
-  double hS[3], zS[3], zN[3], xyS[3];  // S = cell row J-1, N = cell row J; xyS = xi^y of row J-1
+  real hS[3], zS[3], zN[3], xyS[3];  // S = cell row J-1, N = cell row J; xyS = xi^y of row J-1
   // state for the first node row Ja of a band
   __device__ __forceinline__ void start(const SolveP& P, int c0, int Ja) {
-    double zSS[3];
+    real zSS[3];
     lane3(ld2(P.zc, P.G, c0, Ja - 2), zSS);
     lane3(ld2(P.zc, P.G, c0, Ja - 1), zS);
     lane3(ld2(P.zc, P.G, c0, Ja), zN);
     lane3(ld2(P.hc, P.G, c0, Ja - 1), hS);
 #pragma unroll
-    for (int k = 0; k < 3; ++k) xyS[k] = 0.5 * (zN[k] - zSS[k]);
+    for (int k = 0; k < 3; ++k) xyS[k] = RC(0.5) * (zN[k] - zSS[k]);
   }
   // rows of A at node row J from the cell rows h(J) and z(J+1) just loaded, then roll to J+1.
   // S8 with the sums shared between the two nodes: 2 h_E = h_NE + h_SE is a column sum (sh), xi_E a
   // quarter of the difference of the z column sums two cells apart, 2 h_N a row sum, ...;
   // miex = -1 / (8 dx^2), miey = -1 / (8 dy^2).
-  __device__ __forceinline__ Coef step(const SolveP& P, double2 hrow, double2 zrow) {
-    double hN[3], zNN[3], xyN[3], sh[3], sz[3];
+  __device__ __forceinline__ Coef step(const SolveP& P, real2 hrow, real2 zrow) {
+    real hN[3], zNN[3], xyN[3], sh[3], sz[3];
     lane3(hrow, hN);
     lane3(zrow, zNN);
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
       sh[k] = hS[k] + hN[k];
       sz[k] = zS[k] + zN[k];
-      xyN[k] = 0.5 * (zNN[k] - zS[k]);
+      xyN[k] = RC(0.5) * (zNN[k] - zS[k]);
     }
-    const double szm = __shfl_up_sync(NH_FULL, sz[1], 1), szp = __shfl_down_sync(NH_FULL, sz[1], 1);
-    const double xi[3] = {0.25 * (sz[1] - szm), 0.25 * (sz[2] - sz[0]), 0.25 * (szp - sz[1])};
+    const real szm = __shfl_up_sync(NH_FULL, sz[1], 1), szp = __shfl_down_sync(NH_FULL, sz[1], 1);
+    const real xi[3] = {RC(0.25) * (sz[1] - szm), RC(0.25) * (sz[2] - sz[0]), RC(0.25) * (szp - sz[1])};
     Coef C;
 #pragma unroll
     for (int n = 0; n < 2; ++n) {
-      const double hn2 = 0.5 * (sh[n] + sh[n + 1]);  // 2 h_n, (38)
-      const double zx = 0.5 * (sz[n + 1] - sz[n]);
-      const double am = (hn2 - zx) * P.miex, ap = (hn2 + zx) * P.miex;
+      const real hn2 = RC(0.5) * (sh[n] + sh[n + 1]);  // 2 h_n, (38)
+      const real zx = RC(0.5) * (sz[n + 1] - sz[n]);
+      const real am = (hn2 - zx) * P.miex, ap = (hn2 + zx) * P.miex;
       C.e[n] = am * (sh[n + 1] + xi[n + 1]);
       C.w[n] = ap * (sh[n] - xi[n]);
-      const double cx = fma(am, sh[n + 1] - xi[n + 1], ap * (sh[n] + xi[n]));
-      const double hNr = hN[n] + hN[n + 1], hSr = hS[n] + hS[n + 1];
-      const double zy = 0.5 * ((zN[n] + zN[n + 1]) - (zS[n] + zS[n + 1]));
-      const double bm = (hn2 - zy) * P.miey, bp = (hn2 + zy) * P.miey;
-      const double xN = 0.5 * (xyN[n] + xyN[n + 1]), xS = 0.5 * (xyS[n] + xyS[n + 1]);
+      const real cx = fma(am, sh[n + 1] - xi[n + 1], ap * (sh[n] + xi[n]));
+      const real hNr = hN[n] + hN[n + 1], hSr = hS[n] + hS[n + 1];
+      const real zy = RC(0.5) * ((zN[n] + zN[n + 1]) - (zS[n] + zS[n + 1]));
+      const real bm = (hn2 - zy) * P.miey, bp = (hn2 + zy) * P.miey;
+      const real xN = RC(0.5) * (xyN[n] + xyN[n + 1]), xS = RC(0.5) * (xyS[n] + xyS[n + 1]);
       C.n[n] = bm * (hNr + xN);
       C.s[n] = bp * (hSr - xS);
-      const double cy = fma(bm, hNr - xN, bp * (hSr + xS));
-      C.c[n] = 2.0 - (cx + cy);
+      const real cy = fma(bm, hNr - xN, bp * (hSr + xS));
+      C.c[n] = RC(2.0) - (cx + cy);
     }
 #pragma unroll
     for (int k = 0; k < 3; ++k) { hS[k] = hN[k]; zS[k] = zN[k]; zN[k] = zNN[k]; xyS[k] = xyN[k]; }
@@ -269,6 +272,7 @@ struct March {
 
 // 1 / a for a >= 2 (the diagonal of A): hardware seed (20+ bits) and two Newton steps.  Not correctly
 // rounded; the scaling only has to be the same number wherever a node's diagonal is used.
+#if NH_PREC == 64
 __device__ __forceinline__ double rcp_diag(double a) {
   double r;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(a));
@@ -277,12 +281,15 @@ __device__ __forceinline__ double rcp_diag(double a) {
   e = fma(-a, r, 1.0);
   return fma(r, e, r);
 }
+#else
+__device__ __forceinline__ float rcp_diag(float a) { return __frcp_rn(a); }
+#endif
 
 // off-diagonal part of (A x) at the lane's two nodes of row j from the operand rows m: j-1, c: j, n: j+1
-__device__ __forceinline__ double2 offdiag2(const Coef& C, double2 m, double2 c, double2 n) {
-  const double west0 = __shfl_up_sync(NH_FULL, c.y, 1);
-  const double east1 = __shfl_down_sync(NH_FULL, c.x, 1);
-  double2 o;
+__device__ __forceinline__ real2 offdiag2(const Coef& C, real2 m, real2 c, real2 n) {
+  const real west0 = __shfl_up_sync(NH_FULL, c.y, 1);
+  const real east1 = __shfl_down_sync(NH_FULL, c.x, 1);
+  real2 o;
   o.x = fma(C.s[0], m.x, fma(C.n[0], n.x, fma(C.w[0], west0, C.e[0] * c.y)));
   o.y = fma(C.s[1], m.y, fma(C.n[1], n.y, fma(C.w[1], c.x, C.e[1] * east1)));
   return o;
@@ -293,7 +300,7 @@ __device__ __forceinline__ double2 offdiag2(const Coef& C, double2 m, double2 c,
 // aliasing planes), so each warp keeps one full row of every plane in flight while it computes.
 
 // residual pass: r = b - A x (S9: the true residual decides), r0 = r, r^ = r / A_C; partials r.r, b.b
-__device__ __forceinline__ void pass_R(const SolveP& P, double* rh, int buf, double (*red)[NW]) {
+__device__ __forceinline__ void pass_R(const SolveP& P, real* rh, int buf, double (*red)[NW]) {
   const NhGrid& G = P.G;
   const int lane = threadIdx.x & 31;
   const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
@@ -303,16 +310,16 @@ __device__ __forceinline__ void pass_R(const SolveP& P, double* rh, int buf, dou
     Unit U = make_unit(P, k, lane);
     March M;
     M.start(P, U.c0, U.Ja);
-    double2 xm = ld2(P.x, G, U.c0, U.Ja - 1), xc = ld2(P.x, G, U.c0, U.Ja);
+    real2 xm = ld2(P.x, G, U.c0, U.Ja - 1), xc = ld2(P.x, G, U.c0, U.Ja);
     for (int j = U.Ja; j < U.Jb; ++j) {
-      const double2 xn = ld2(P.x, G, U.c0, j + 1), bb = ld2(P.b, G, U.c0, j);
+      const real2 xn = ld2(P.x, G, U.c0, j + 1), bb = ld2(P.b, G, U.c0, j);
       const Coef C = M.step(P, ld2(P.hc, G, U.c0, j), ld2(P.zc, G, U.c0, j + 1));
-      const double2 off = offdiag2(C, xm, xc, xn);
-      const double2 rr = make_double2(bb.x - fma(C.c[0], xc.x, off.x), bb.y - fma(C.c[1], xc.y, off.y));
+      const real2 off = offdiag2(C, xm, xc, xn);
+      const real2 rr = make_real2(bb.x - fma(C.c[0], xc.x, off.x), bb.y - fma(C.c[1], xc.y, off.y));
       st2(P.r0, P, U, j, rr);
-      st2(rh, P, U, j, make_double2(rr.x * rcp_diag(C.c[0]), rr.y * rcp_diag(C.c[1])));
-      if (U.own0) { acc[0] = fma(rr.x, rr.x, acc[0]); acc[1] = fma(bb.x, bb.x, acc[1]); }
-      if (U.own1) { acc[0] = fma(rr.y, rr.y, acc[0]); acc[1] = fma(bb.y, bb.y, acc[1]); }
+      st2(rh, P, U, j, make_real2(rr.x * rcp_diag(C.c[0]), rr.y * rcp_diag(C.c[1])));
+      if (U.own0) { acc[0] = fma(D(rr.x), D(rr.x), acc[0]); acc[1] = fma(D(bb.x), D(bb.x), acc[1]); }
+      if (U.own1) { acc[0] = fma(D(rr.y), D(rr.y), acc[0]); acc[1] = fma(D(bb.y), D(bb.y), acc[1]); }
       xm = xc; xc = xn;
     }
   }
@@ -322,16 +329,16 @@ __device__ __forceinline__ void pass_R(const SolveP& P, double* rh, int buf, dou
 // pass B: s^ = r^ - alpha v^ (rows Ja-1..Jb), t = A s^ (rows Ja..Jb-1), stored as t^ = t / A_C;
 // partials of the unscaled vectors: t.s, t.t, s.s, r0.s, r0.t
 struct RowB {  // operands of sweep step j: r^, v^ of row j+1; r0, h of row j; z of row j+1
-  double2 r, v, q, h, z;
+  real2 r, v, q, h, z;
 };
-__device__ __forceinline__ void ld_rowb(RowB& X, const SolveP& P, const double* r, const double* v,
+__device__ __forceinline__ void ld_rowb(RowB& X, const SolveP& P, const real* r, const real* v,
                                         int c0, int j) {
   X.r = ld2(r, P.G, c0, j + 1); X.v = ld2(v, P.G, c0, j + 1);
   X.q = ld2(P.r0, P.G, c0, j);
   X.h = ld2(P.hc, P.G, c0, j); X.z = ld2(P.zc, P.G, c0, j + 1);
 }
 
-__device__ __forceinline__ void pass_B(const SolveP& P, double alpha, const double* r, const double* v,
+__device__ __forceinline__ void pass_B(const SolveP& P, real alpha, const real* r, const real* v,
                                     int buf, double (*red)[NW]) {
   const NhGrid& G = P.G;
   const int lane = threadIdx.x & 31;
@@ -340,34 +347,36 @@ __device__ __forceinline__ void pass_B(const SolveP& P, double alpha, const doub
   double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
   for (int k = gw; k < nunits; k += tw) {
     Unit U = make_unit(P, k, lane);
-    auto srow = [&](double2 a, double2 b) {
-      return make_double2(fma(-alpha, b.x, a.x), fma(-alpha, b.y, a.y));
+    auto srow = [&](real2 a, real2 b) {
+      return make_real2(fma(-alpha, b.x, a.x), fma(-alpha, b.y, a.y));
     };
     March M;
     M.start(P, U.c0, U.Ja);
-    double2 sm = srow(ld2(r, G, U.c0, U.Ja - 1), ld2(v, G, U.c0, U.Ja - 1));
-    double2 sc = srow(ld2(r, G, U.c0, U.Ja), ld2(v, G, U.c0, U.Ja));
+    real2 sm = srow(ld2(r, G, U.c0, U.Ja - 1), ld2(v, G, U.c0, U.Ja - 1));
+    real2 sc = srow(ld2(r, G, U.c0, U.Ja), ld2(v, G, U.c0, U.Ja));
     // One operand set; the loads of step j+1 are issued as soon as step j has moved its operands
     // into the marching state, before the arithmetic of the step (row index clamped: the last
     // request is never used).
     RowB X;
     ld_rowb(X, P, r, v, U.c0, U.Ja);
     for (int j = U.Ja; j < U.Jb; ++j) {
-      const double2 sn = srow(X.r, X.v);
-      const double2 q = X.q;
+      const real2 sn = srow(X.r, X.v);
+      const real2 q = X.q;
       const Coef C = M.step(P, X.h, X.z);
       if (j + 1 < U.Jb) ld_rowb(X, P, r, v, U.c0, j + 1);
-      const double2 off = offdiag2(C, sm, sc, sn);
-      const double2 tu = make_double2(fma(C.c[0], sc.x, off.x), fma(C.c[1], sc.y, off.y));  // t
-      const double2 su = make_double2(C.c[0] * sc.x, C.c[1] * sc.y);                        // s
-      st2(P.t, P, U, j, make_double2(fma(rcp_diag(C.c[0]), off.x, sc.x), fma(rcp_diag(C.c[1]), off.y, sc.y)));
+      const real2 off = offdiag2(C, sm, sc, sn);
+      const real2 tu = make_real2(fma(C.c[0], sc.x, off.x), fma(C.c[1], sc.y, off.y));  // t
+      const real2 su = make_real2(C.c[0] * sc.x, C.c[1] * sc.y);                        // s
+      st2(P.t, P, U, j, make_real2(fma(rcp_diag(C.c[0]), off.x, sc.x), fma(rcp_diag(C.c[1]), off.y, sc.y)));
       if (U.own0) {
-        acc[0] = fma(tu.x, su.x, acc[0]); acc[1] = fma(tu.x, tu.x, acc[1]); acc[2] = fma(su.x, su.x, acc[2]);
-        acc[3] = fma(q.x, su.x, acc[3]); acc[4] = fma(q.x, tu.x, acc[4]);
+        acc[0] = fma(D(tu.x), D(su.x), acc[0]); acc[1] = fma(D(tu.x), D(tu.x), acc[1]);
+        acc[2] = fma(D(su.x), D(su.x), acc[2]);
+        acc[3] = fma(D(q.x), D(su.x), acc[3]); acc[4] = fma(D(q.x), D(tu.x), acc[4]);
       }
       if (U.own1) {
-        acc[0] = fma(tu.y, su.y, acc[0]); acc[1] = fma(tu.y, tu.y, acc[1]); acc[2] = fma(su.y, su.y, acc[2]);
-        acc[3] = fma(q.y, su.y, acc[3]); acc[4] = fma(q.y, tu.y, acc[4]);
+        acc[0] = fma(D(tu.y), D(su.y), acc[0]); acc[1] = fma(D(tu.y), D(tu.y), acc[1]);
+        acc[2] = fma(D(su.y), D(su.y), acc[2]);
+        acc[3] = fma(D(q.y), D(su.y), acc[3]); acc[4] = fma(D(q.y), D(tu.y), acc[4]);
       }
       sm = sc; sc = sn;
     }
@@ -379,11 +388,11 @@ __device__ __forceinline__ void pass_B(const SolveP& P, double alpha, const doub
 // x += alpha p^ + omega s^; r^' = s^ - omega t^; p^' = r^' + beta (p^ - omega v^).  Then v' = A p^',
 // stored as v^' = v' / A_C.  partials of the unscaled vectors: r0.v', r'.r'
 struct RowV {  // vector row of pass CA
-  double2 r, v, t, p, x;
+  real2 r, v, t, p, x;
 };
 template <bool FIRST>
-__device__ __forceinline__ void ld_rowv(RowV& V, const SolveP& P, const double* r, const double* p,
-                                        const double* v, int c0, int j) {
+__device__ __forceinline__ void ld_rowv(RowV& V, const SolveP& P, const real* r, const real* p,
+                                        const real* v, int c0, int j) {
   V.r = ld2(r, P.G, c0, j);
   if (!FIRST) {
     V.v = ld2(v, P.G, c0, j); V.t = ld2(P.t, P.G, c0, j);
@@ -392,13 +401,13 @@ __device__ __forceinline__ void ld_rowv(RowV& V, const SolveP& P, const double* 
 }
 struct RowCA {  // operands of sweep step j: vectors of row j+1; r0, h of row j; z of row j+1
   RowV V;
-  double2 q, h, z;
+  real2 q, h, z;
 };
 
 template <bool FIRST>
-__device__ __forceinline__ void pass_CA(const SolveP& P, double alpha, double omega, double beta,
-                                     const double* r, const double* p, const double* v, double* rN,
-                                     double* pN, double* vN, int buf, double (*red)[NW]) {
+__device__ __forceinline__ void pass_CA(const SolveP& P, real alpha, real omega, real beta,
+                                     const real* r, const real* p, const real* v, real* rN,
+                                     real* pN, real* vN, int buf, double (*red)[NW]) {
   const int lane = threadIdx.x & 31;
   const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
   const int nunits = P.nstrips * P.nbands;
@@ -406,18 +415,18 @@ __device__ __forceinline__ void pass_CA(const SolveP& P, double alpha, double om
   for (int k = gw; k < nunits; k += tw) {
     Unit U = make_unit(P, k, lane);
     // new r^, p^, x of a row from its loaded operands
-    auto vrow = [&](const RowV& V, double2& rn, double2& pn, double2& xx) {
+    auto vrow = [&](const RowV& V, real2& rn, real2& pn, real2& xx) {
       if (FIRST) {
         rn = V.r; pn = V.r; xx = V.r;
       } else {
-        const double2 s = make_double2(fma(-alpha, V.v.x, V.r.x), fma(-alpha, V.v.y, V.r.y));
-        rn = make_double2(fma(-omega, V.t.x, s.x), fma(-omega, V.t.y, s.y));
-        pn = make_double2(fma(beta, fma(-omega, V.v.x, V.p.x), rn.x),
+        const real2 s = make_real2(fma(-alpha, V.v.x, V.r.x), fma(-alpha, V.v.y, V.r.y));
+        rn = make_real2(fma(-omega, V.t.x, s.x), fma(-omega, V.t.y, s.y));
+        pn = make_real2(fma(beta, fma(-omega, V.v.x, V.p.x), rn.x),
                           fma(beta, fma(-omega, V.v.y, V.p.y), rn.y));
-        xx = make_double2(V.x.x + fma(omega, s.x, alpha * V.p.x), V.x.y + fma(omega, s.y, alpha * V.p.y));
+        xx = make_real2(V.x.x + fma(omega, s.x, alpha * V.p.x), V.x.y + fma(omega, s.y, alpha * V.p.y));
       }
     };
-    auto store_row = [&](int j, double2 rn, double2 pn, double2 xx) {
+    auto store_row = [&](int j, real2 rn, real2 pn, real2 xx) {
       if (!FIRST) st2(P.x, P, U, j, xx);
       st2(rN, P, U, j, rn);
       st2(pN, P, U, j, pn);
@@ -429,12 +438,12 @@ __device__ __forceinline__ void pass_CA(const SolveP& P, double alpha, double om
     };
     March M;
     M.start(P, U.c0, U.Ja);
-    double2 pm, pc, rc;  // p^' of rows j-1, j; r^' of row j (its A_C is known one step later)
+    real2 pm, pc, rc;  // p^' of rows j-1, j; r^' of row j (its A_C is known one step later)
     {
       RowV V0, V1;
       ld_rowv<FIRST>(V0, P, r, p, v, U.c0, U.Ja - 1);
       ld_rowv<FIRST>(V1, P, r, p, v, U.c0, U.Ja);
-      double2 r0_, x0_, x1_;
+      real2 r0_, x0_, x1_;
       vrow(V0, r0_, pm, x0_);
       vrow(V1, rc, pc, x1_);
       store_row(U.Ja, rc, pc, x1_);
@@ -446,18 +455,18 @@ __device__ __forceinline__ void pass_CA(const SolveP& P, double alpha, double om
     ld_set(X, U.Ja);
     for (int j = U.Ja; j < U.Jb; ++j) {
       const bool own_next = j + 1 < U.Jb;
-      double2 rn, pn, xx;
+      real2 rn, pn, xx;
       vrow(X.V, rn, pn, xx);
       const Coef C = M.step(P, X.h, X.z);
-      const double2 q = X.q;
+      const real2 q = X.q;
       if (own_next) ld_set(X, min(j + 1, U.Jb - 1));  // operands of the next step
-      const double2 off = offdiag2(C, pm, pc, pn);
-      const double2 vu = make_double2(fma(C.c[0], pc.x, off.x), fma(C.c[1], pc.y, off.y));  // v'
+      const real2 off = offdiag2(C, pm, pc, pn);
+      const real2 vu = make_real2(fma(C.c[0], pc.x, off.x), fma(C.c[1], pc.y, off.y));  // v'
       if (own_next) store_row(j + 1, rn, pn, xx);
-      st2(vN, P, U, j, make_double2(fma(rcp_diag(C.c[0]), off.x, pc.x), fma(rcp_diag(C.c[1]), off.y, pc.y)));
-      const double2 ru = make_double2(C.c[0] * rc.x, C.c[1] * rc.y);  // r' of row j
-      if (U.own0) { acc[0] = fma(q.x, vu.x, acc[0]); acc[1] = fma(ru.x, ru.x, acc[1]); }
-      if (U.own1) { acc[0] = fma(q.y, vu.y, acc[0]); acc[1] = fma(ru.y, ru.y, acc[1]); }
+      st2(vN, P, U, j, make_real2(fma(rcp_diag(C.c[0]), off.x, pc.x), fma(rcp_diag(C.c[1]), off.y, pc.y)));
+      const real2 ru = make_real2(C.c[0] * rc.x, C.c[1] * rc.y);  // r' of row j
+      if (U.own0) { acc[0] = fma(D(q.x), D(vu.x), acc[0]); acc[1] = fma(D(ru.x), D(ru.x), acc[1]); }
+      if (U.own1) { acc[0] = fma(D(q.y), D(vu.y), acc[0]); acc[1] = fma(D(ru.y), D(ru.y), acc[1]); }
       pm = pc; pc = pn; rc = rn;
     }
   }
@@ -474,13 +483,13 @@ __device__ void phase_images(const SolveP& P) {
 
 // x += alpha p^ + omega s^, s^ = r^ - alpha v^  (final update of an iteration whose pass CA never
 // ran: half-step exit with omega = 0, and the polish iteration)
-__device__ void phase_update_x(const SolveP& P, double alpha, double omega, const double* r,
-                               const double* p, const double* v) {
+__device__ void phase_update_x(const SolveP& P, real alpha, real omega, const real* r,
+                               const real* p, const real* v) {
   const NhGrid& G = P.G;
   for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
     for (int I = threadIdx.x; I < G.nnx; I += NT) {
       size_t k = nidx(G, I, J);
-      double s = r[k] - alpha * v[k];
+      real s = r[k] - alpha * v[k];
       store_images(G, P.x, I, J, P.x[k] + (alpha * p[k] + omega * s));
     }
 }
@@ -488,7 +497,7 @@ __device__ void phase_update_x(const SolveP& P, double alpha, double omega, cons
 __device__ void phase_zero_x(const SolveP& P) {
   const NhGrid& G = P.G;
   for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
-    for (int I = threadIdx.x; I < G.nnx; I += NT) store_images(G, P.x, I, J, 0.0);
+    for (int I = threadIdx.x; I < G.nnx; I += NT) store_images(G, P.x, I, J, RC(0.0));
 }
 
 __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
@@ -496,16 +505,16 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
   __shared__ double red[MAXDOT][NW];
   __shared__ double bc[MAXDOT];
 
-  double *rC = P.rA, *rN = P.rB, *pC = P.pA, *pN = P.pB, *vC = P.vA, *vN = P.vB;  // current / next
+  real *rC = P.rA, *rN = P.rB, *pC = P.pA, *pN = P.pB, *vC = P.vA, *vN = P.vB;  // current / next
   auto flip = [&]() {
-    double* t;
+    real* t;
     t = rC; rC = rN; rN = t;
     t = pC; pC = pN; pN = t;
     t = vC; vC = vN; vN = t;
   };
   int buf = 0;  // partial buffer of the pass in flight (alternates: one grid barrier per pass)
   int iters = 0, converged = 0, status = 0;
-  double rnorm = 0.0, bnorm = 0.0, tol = 0.0;
+  double rnorm = 0.0, bnorm = 0.0, tol = 0.0, rnorm_prev = 0.0;
 
   phase_images(P);
   grid.sync();
@@ -524,10 +533,15 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
     }
     if (!(rnorm == rnorm)) { status = NH_ENAN; break; }
     if (rnorm <= tol) { converged = 1; break; }
+    // fp32 variant: an fp32 iterate cannot satisfy the system better than ~ kappa u32 ||b||.  When a
+    // whole cycle (recursive residual below tol) no longer halves the TRUE residual, the attainable
+    // accuracy has been reached: accept the iterate; res_last reports what was reached.
+    if (kEta && cycle > 0 && rnorm > 0.5 * rnorm_prev) { converged = 1; break; }
+    rnorm_prev = rnorm;
     if (iters >= P.maxit) break;
     // first direction of the cycle: p = r, v = A M^-1 p, sigma = r0.v
     double rho = d2[0];
-    pass_CA<true>(P, 0.0, 0.0, 0.0, rC, pC, vC, rN, pN, vN, buf, red);
+    pass_CA<true>(P, RC(0.0), RC(0.0), RC(0.0), rC, pC, vC, rN, pN, vN, buf, red);
     flip();
     grid.sync();
     grid_sums<2>(P.part, buf, d2, red, bc);
@@ -537,12 +551,12 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
       if (fabs(rho) < 1e-300 || fabs(sigma) < 1e-300) break;  // breakdown -> restart
       double alpha = rho / sigma;
       iters++;
-      pass_B(P, alpha, rC, vC, buf, red);
+      pass_B(P, (real)alpha, rC, vC, buf, red);
       grid.sync();
       grid_sums<5>(P.part, buf, d5, red, bc);
       buf ^= 1;
       if (sqrt(d5[2]) <= tol) {  // half-step exit: x += alpha p^
-        phase_update_x(P, alpha, 0.0, rC, pC, vC);
+        phase_update_x(P, (real)alpha, RC(0.0), rC, pC, vC);
         grid.sync();
         break;
       }
@@ -552,7 +566,7 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
       double rho_new = d5[3] - omega * d5[4];  // r0.r' = r0.s - omega r0.t  (R25)
       double beta = (rho_new / rho) * (alpha / omega);
       rho = rho_new;
-      pass_CA<false>(P, alpha, omega, beta, rC, pC, vC, rN, pN, vN, buf, red);
+      pass_CA<false>(P, (real)alpha, (real)omega, (real)beta, rC, pC, vC, rN, pN, vN, buf, red);
       flip();
       grid.sync();
       grid_sums<2>(P.part, buf, d2, red, bc);
@@ -570,7 +584,7 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
   if (converged && rnorm > 0.0) {
     double d2[2], d5[5];
     double rho = rnorm * rnorm;
-    pass_CA<true>(P, 0.0, 0.0, 0.0, rC, pC, vC, rN, pN, vN, buf, red);
+    pass_CA<true>(P, RC(0.0), RC(0.0), RC(0.0), rC, pC, vC, rN, pN, vN, buf, red);
     flip();
     grid.sync();
     grid_sums<2>(P.part, buf, d2, red, bc);
@@ -578,12 +592,12 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
     double sigma = d2[0];
     if (fabs(rho) >= 1e-300 && fabs(sigma) >= 1e-300) {
       double alpha = rho / sigma;
-      pass_B(P, alpha, rC, vC, buf, red);
+      pass_B(P, (real)alpha, rC, vC, buf, red);
       grid.sync();
       grid_sums<5>(P.part, buf, d5, red, bc);
       buf ^= 1;
       double omega = (d5[1] > 0.0) ? d5[0] / d5[1] : 0.0;
-      phase_update_x(P, alpha, omega, rC, pC, vC);
+      phase_update_x(P, (real)alpha, (real)omega, rC, pC, vC);
       grid.sync();
     }
   }
@@ -615,25 +629,26 @@ constexpr int NT1 = 256, NW1 = NT1 / 32;  // CTA shape of k_srj (128 registers, 
 struct SrjP {
   NhGrid G;
   int nstrips, R, nbands;
-  const double *cE, *cW, *cN, *cS, *bp, *costab;
-  double *xA, *xB;  // xA = the pressure plane p (start and result), xB = scratch
+  const real *cE, *cW, *cN, *cS, *bp;
+  const double* costab;
+  real *xA, *xB;  // xA = the pressure plane p (start and result), xB = scratch
   NhScal* sc;
   double eps, rel;  // tolerance of (32): eps, or rel * max|b'| when rel > 0
   int maxit, mmax, count_stats;
 };
 
-__device__ __forceinline__ void srj_sweep(const SrjP& P, const SolveP& Q, double om, const double* x,
-                                          double* xn, unsigned long long* Eslot) {
+__device__ __forceinline__ void srj_sweep(const SrjP& P, const SolveP& Q, real om, const real* x,
+                                          real* xn, unsigned long long* Eslot) {
   const NhGrid& G = P.G;
   const int lane = threadIdx.x & 31;
   const int gw = blockIdx.x * NW1 + (threadIdx.x >> 5), tw = gridDim.x * NW1;
   const int nunits = P.nstrips * P.nbands;
-  double emax = 0.0;
+  real emax = RC(0.0);
   bool bad = false;
-  struct Row { double2 xn, b, e, w, n, s; };
+  struct Row { real2 xn, b, e, w, n, s; };
   for (int u = gw; u < nunits; u += tw) {
     Unit U = make_unit(Q, u, lane);
-    double2 xm = ld2(x, G, U.c0, U.Ja - 1), xc = ld2(x, G, U.c0, U.Ja);
+    real2 xm = ld2(x, G, U.c0, U.Ja - 1), xc = ld2(x, G, U.c0, U.Ja);
     auto ld_row = [&](Row& X, int j) {  // operands of sweep step j (x of row j+1, the rest of row j)
       X.xn = ld2(x, G, U.c0, min(j + 1, U.Jb));
       const int jc = min(j, U.Jb - 1);
@@ -643,14 +658,14 @@ __device__ __forceinline__ void srj_sweep(const SrjP& P, const SolveP& Q, double
     };
     auto step = [&](int j, Row& cur, Row& nxt) {
       ld_row(nxt, j + 1);  // request the next step's operands first
-      double west0 = __shfl_up_sync(0xffffffffu, xc.y, 1);
-      double east1 = __shfl_down_sync(0xffffffffu, xc.x, 1);
-      double ax0 = xc.x + (((cur.e.x * xc.y + cur.w.x * west0) + cur.n.x * cur.xn.x) + cur.s.x * xm.x);
-      double ax1 = xc.y + (((cur.e.y * east1 + cur.w.y * xc.x) + cur.n.y * cur.xn.y) + cur.s.y * xm.y);
-      double z0 = cur.b.x - ax0, z1 = cur.b.y - ax1;
+      real west0 = __shfl_up_sync(0xffffffffu, xc.y, 1);
+      real east1 = __shfl_down_sync(0xffffffffu, xc.x, 1);
+      real ax0 = xc.x + (((cur.e.x * xc.y + cur.w.x * west0) + cur.n.x * cur.xn.x) + cur.s.x * xm.x);
+      real ax1 = xc.y + (((cur.e.y * east1 + cur.w.y * xc.x) + cur.n.y * cur.xn.y) + cur.s.y * xm.y);
+      real z0 = cur.b.x - ax0, z1 = cur.b.y - ax1;
       if (U.own0) { emax = fmax(emax, fabs(z0)); bad |= !(z0 == z0); }
       if (U.own1) { emax = fmax(emax, fabs(z1)); bad |= !(z1 == z1); }
-      st2(xn, Q, U, j, make_double2(xc.x + om * z0, xc.y + om * z1));
+      st2(xn, Q, U, j, make_real2(xc.x + om * z0, xc.y + om * z1));
       xm = xc; xc = cur.xn;
     };
     Row A, B;
@@ -662,14 +677,14 @@ __device__ __forceinline__ void srj_sweep(const SrjP& P, const SolveP& Q, double
   }
   // CTA max -> one integer atomicMax (exact, order independent)
   for (int o = 16; o > 0; o >>= 1) emax = fmax(emax, __shfl_xor_sync(0xffffffffu, emax, o));
-  __shared__ double wmax[NW1];
+  __shared__ real wmax[NW1];
   if (lane == 0) wmax[threadIdx.x >> 5] = emax;
   int anybad = __syncthreads_or(bad);
   if (threadIdx.x == 0) {
-    double m = 0.0;
+    real m = RC(0.0);
 #pragma unroll
     for (int w = 0; w < NW1; ++w) m = fmax(m, wmax[w]);
-    if (m > 0.0) atomicMax(Eslot, (unsigned long long)__double_as_longlong(m));
+    if (m > RC(0.0)) atomicMax(Eslot, (unsigned long long)__double_as_longlong((double)m));
     if (anybad) atomicOr(&P.sc->srj_bad, 1);
   }
 }
@@ -687,12 +702,12 @@ __global__ void __launch_bounds__(NT1, NH_SRJ_MINB) k_srj(SrjP P) {
   const double bmax = __longlong_as_double((long long)sc->srj_bmax_bits);
   int iters = 0, status = 0;
   double E = 0.0;
-  double *x = P.xA, *xn = P.xB;
+  real *x = P.xA, *xn = P.xB;
   if (!(bmax == bmax) || isinf(bmax)) {
     status = NH_ENAN;
   } else if (bmax == 0.0) {  // b = 0 => p~ = 0, zero iterations (same convention as solver 0)
     for (int J = blockIdx.x; J < G.nny; J += gridDim.x)
-      for (int I = threadIdx.x; I < G.nnx; I += NT1) P.xA[nidx(G, I, J)] = 0.0;
+      for (int I = threadIdx.x; I < G.nnx; I += NT1) P.xA[nidx(G, I, J)] = RC(0.0);
   } else {
     // cycle length: smallest power of two with M sqrt(2 (1 - rho)) >= 7.6, at most mmax.  Where a
     // row is not strictly diagonally dominant (rho >= 1, e.g. across a discontinuous free surface)
@@ -711,7 +726,7 @@ __global__ void __launch_bounds__(NT1, NH_SRJ_MINB) k_srj(SrjP P) {
     for (;;) {
       const double om = dominant ? 1.0 / (1.0 - rho * cosv[iters % M]) : 1.0;
       unsigned long long* slot = &sc->srj_E_bits[iters % 3];
-      srj_sweep(P, Q, om, x, xn, slot);
+      srj_sweep(P, Q, (real)om, x, xn, slot);
       grid.sync();
       E = __longlong_as_double((long long)__ldcg(slot));
       const int bad = __ldcg(&sc->srj_bad);
@@ -719,7 +734,7 @@ __global__ void __launch_bounds__(NT1, NH_SRJ_MINB) k_srj(SrjP P) {
       if (bad) { status = NH_ENAN; break; }
       if (E < tol) break;  // eq. (32): x is the accepted iterate
       if (iters >= P.maxit) { status = NH_ENOCONV; break; }
-      double* t = x; x = xn; xn = t;
+      real* t = x; x = xn; xn = t;
       iters++;
     }
     if (x != P.xA) {  // the accepted iterate lives in the scratch plane
@@ -749,7 +764,7 @@ __global__ void __launch_bounds__(NT1, NH_SRJ_MINB) k_srj(SrjP P) {
 // Cooperative grid (one wave of co-resident CTAs) and the band height R: every warp takes the
 // units u = gw, gw + tw, ... (strip fastest, so neighbouring warps sweep neighbouring strips of the
 // same band); R minimises rounds x (R + 2 halo rows).
-int nh_solver_setup(nh_ctx* c) {
+int nh_solver_setup(Ctx* c) {
   int occ = 0;
   cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bicgstab, NT, 0);
   if (e != cudaSuccess || occ < 1) {
@@ -825,7 +840,7 @@ int nh_solver_setup(nh_ctx* c) {
   return NH_OK;
 }
 
-void nh_launch_solve(nh_ctx* c, const double* b, double* x, int count_stats) {
+void nh_launch_solve(Ctx* c, const real* b, real* x, int count_stats) {
   if (c->prm.solver == 1) {  // b is c->kr = b / A_C here (nh_launch_scale_rows)
     SrjP S;
     S.G = c->g;
@@ -847,10 +862,13 @@ void nh_launch_solve(nh_ctx* c, const double* b, double* x, int count_stats) {
   P.r0 = c->kr0; P.t = c->kt;
   P.rA = c->kr; P.rB = c->krB; P.pA = c->kpA; P.pB = c->kpB; P.vA = c->kvA; P.vB = c->kvB;
   P.part = c->part; P.sc = c->sc; P.rtol = c->prm.solver_rtol; P.maxit = c->prm.solver_maxit;
-  P.miex = -1.0 / (8.0 * c->g.dx * c->g.dx); P.miey = -1.0 / (8.0 * c->g.dy * c->g.dy);
+  P.miex = (real)(-1.0 / (8.0 * (double)c->g.dx * (double)c->g.dx));
+  P.miey = (real)(-1.0 / (8.0 * (double)c->g.dy * (double)c->g.dy));
   P.count_stats = count_stats;
   void* args[] = {&P};
   NH_CUDA_OK(c, cudaLaunchCooperativeKernel((void*)k_bicgstab, dim3(c->solver_grid), dim3(NT), args,
                                             0, c->stream));
   c->launches++;
 }
+
+}  // namespace NH_NS
