@@ -444,7 +444,7 @@ def test_manning_beach_reduced_parity(O, G):
     # config 4 with the paper's run-up roughness n = 0.01 (L631), reduced size.  The friction factor
     # 1 / (1 + dt g n^2 |u| / h^(4/3)) of a thin film (h ~ 1e-5) turns solver-level differences into
     # O(1e-6) differences of q within 50 steps: two ORACLE runs at solver_rtol 1e-12 and 1e-13 differ by
-    # 3.7e3 bars at step 75 (profiles/r02b_config4_sensitivity.md).  Compared over the wave's arrival
+    # 1e3 bars at step 60 (profiles/r02b_config4_sensitivity.md, addendum).  Compared over the wave's arrival
     # with the paper's solver (solver 1: both sides do the same arithmetic, the cube root of h^(4/3)
     # included, R31: bit for bit), and with the default solver over a window short of that amplification.
     cfg = inputs.make_config(4, nx=512, ny=8)
