@@ -2,7 +2,7 @@
  *
  * One time step of the scheme of arXiv 1706.04551, written step by step in the
  * paper's order and notation.  Steps S0..S11 and readings R1..R23 refer to SURVEY.md 8(c)
- * (restated in DESIGN.md); "L<n>" are PAPER.md line numbers.
+ * (restated in DESIGN.md; R24..R31 are DESIGN.md's own); "L<n>" are PAPER.md line numbers.
  *
  * Plain C, fp64, scalar loops, no blocking / fusion / reordering beyond what the formulas
  * state.  OpenMP only splits loops over rows j (every row is independent inside a loop).
@@ -12,9 +12,12 @@
  * Stoker dam break (P3), printed 1D coefficients (43) + x<->y symmetry (P4), constraint after
  * correction via an independent transcription of (36)-(41) (P5), dense LU (P6), dry-slope
  * closed form (P7), linear dispersion relation (P8), 2nd-order convergence (P9), diagonal
- * dominance (P10), flat-bottom symmetry (P11), breaking properties (P12).
- * Parity unpinned (internal consistency only): the 3-component 2D face solver reading R3,
- * the 2D breaking reading R12/R13, the relaxation-zone reading R18.
+ * dominance (P10), flat-bottom symmetry (P11), breaking properties and the printed 1D magnitudes
+ * (P12), closed forms of the generating / absorbing zones (R18, R29), of the CFL time step (23), of
+ * Manning friction (R27) and of the w transport (R30), the all-dry branch (R26), the fixed-algorithm
+ * cube root and sech^2 against libm (R31).
+ * Parity unpinned (internal consistency only): the 3-component 2D face solver reading R3 and the
+ * 2D extension R12 of the breaking terms.
  */
 #include "nh_oracle.h"
 #include <math.h>
