@@ -83,7 +83,7 @@ struct SolveP {
   double* part;  // [2][MAXDOT][gridDim.x]
   NhScal* sc;
   double rtol;
-  real miex, miey;  // -1 / (8 dx^2), -1 / (8 dy^2)
+  real mx2, my2;  // -1 / (16 dx^2), -1 / (16 dy^2)
   int maxit;
   int count_stats;
 };
@@ -219,7 +219,11 @@ __device__ __forceinline__ void lane3(real2 own, real (&q)[3]) {
   q[0] = own.x; q[1] = own.y; q[2] = __shfl_down_sync(NH_FULL, own.x, 1);
 }
 struct March {
-  real hS[3], zS[3], zN[3], xyS[3];  // S = cell row J-1, N = cell row J; xyS = xi^y of row J-1
+  // S = cell row J-1, N = cell row J.  Carried between sweep steps: the raw rows h(J-1), z(J-1), z(J)
+  // (column sums), and the row-pair sums of row J-1 at the lane's two nodes (they were the "north"
+  // sums of the previous step): h, z, and dz2 = z(J) - z(J-2) = 2 xi^y of row J-1.
+  real hS[3], zS[3], zN[3];
+  real hSr[2], zSr[2], tS[2];
   // state for the first node row Ja of a band
   __device__ __forceinline__ void start(const SolveP& P, int c0, int Ja) {
     real zSS[3];
@@ -228,44 +232,47 @@ struct March {
     lane3(ld2(P.zc, P.G, c0, Ja), zN);
     lane3(ld2(P.hc, P.G, c0, Ja - 1), hS);
 #pragma unroll
-    for (int k = 0; k < 3; ++k) xyS[k] = RC(0.5) * (zN[k] - zSS[k]);
+    for (int n = 0; n < 2; ++n) {
+      hSr[n] = hS[n] + hS[n + 1];
+      zSr[n] = zS[n] + zS[n + 1];
+      tS[n] = (zN[n] - zSS[n]) + (zN[n + 1] - zSS[n + 1]);
+    }
   }
   // rows of A at node row J from the cell rows h(J) and z(J+1) just loaded, then roll to J+1.
-  // S8 with the sums shared between the two nodes: 2 h_E = h_NE + h_SE is a column sum (sh), xi_E a
-  // quarter of the difference of the z column sums two cells apart, 2 h_N a row sum, ...;
-  // miex = -1 / (8 dx^2), miey = -1 / (8 dy^2).
+  // S8 with the sums shared between the two nodes and the factors 1/2, 1/4 folded into the
+  // multipliers: 2 h_E = h_NE + h_SE is a column sum (sh), 4 xi_E the difference of the z column
+  // sums two cells apart, 2 h_N a row sum, 4 xi_N the row-pair sum of z(J+1) - z(J-1);
+  // mx2 = -1 / (16 dx^2), my2 = -1 / (16 dy^2).
   __device__ __forceinline__ Coef step(const SolveP& P, real2 hrow, real2 zrow) {
-    real hN[3], zNN[3], xyN[3], sh[3], sz[3];
+    real hN[3], zNN[3], sh[3], sz[3];
     lane3(hrow, hN);
     lane3(zrow, zNN);
 #pragma unroll
-    for (int k = 0; k < 3; ++k) {
-      sh[k] = hS[k] + hN[k];
-      sz[k] = zS[k] + zN[k];
-      xyN[k] = RC(0.5) * (zNN[k] - zS[k]);
-    }
+    for (int k = 0; k < 3; ++k) { sh[k] = hS[k] + hN[k]; sz[k] = zS[k] + zN[k]; }
     const real szm = __shfl_up_sync(NH_FULL, sz[1], 1), szp = __shfl_down_sync(NH_FULL, sz[1], 1);
-    const real xi[3] = {RC(0.25) * (sz[1] - szm), RC(0.25) * (sz[2] - sz[0]), RC(0.25) * (szp - sz[1])};
+    const real x4[3] = {sz[1] - szm, sz[2] - sz[0], szp - sz[1]};  // 4 xi of the three cell columns
+    const real q = RC(0.25);
     Coef C;
 #pragma unroll
     for (int n = 0; n < 2; ++n) {
-      const real hn2 = RC(0.5) * (sh[n] + sh[n + 1]);  // 2 h_n, (38)
-      const real zx = RC(0.5) * (sz[n + 1] - sz[n]);
-      const real am = (hn2 - zx) * P.miex, ap = (hn2 + zx) * P.miex;
-      C.e[n] = am * (sh[n + 1] + xi[n + 1]);
-      C.w[n] = ap * (sh[n] - xi[n]);
-      const real cx = fma(am, sh[n + 1] - xi[n + 1], ap * (sh[n] + xi[n]));
-      const real hNr = hN[n] + hN[n + 1], hSr = hS[n] + hS[n + 1];
-      const real zy = RC(0.5) * ((zN[n] + zN[n + 1]) - (zS[n] + zS[n + 1]));
-      const real bm = (hn2 - zy) * P.miey, bp = (hn2 + zy) * P.miey;
-      const real xN = RC(0.5) * (xyN[n] + xyN[n + 1]), xS = RC(0.5) * (xyS[n] + xyS[n + 1]);
-      C.n[n] = bm * (hNr + xN);
-      C.s[n] = bp * (hSr - xS);
-      const real cy = fma(bm, hNr - xN, bp * (hSr + xS));
+      const real a = sh[n] + sh[n + 1];   // 4 h_n, (38)
+      const real bx = sz[n + 1] - sz[n];  // 2 (z_E - z_W)
+      const real am = (a - bx) * P.mx2, ap = (a + bx) * P.mx2;
+      C.e[n] = am * fma(q, x4[n + 1], sh[n + 1]);
+      C.w[n] = ap * fma(-q, x4[n], sh[n]);
+      const real cx = fma(am, fma(-q, x4[n + 1], sh[n + 1]), ap * fma(q, x4[n], sh[n]));
+      const real hNr = hN[n] + hN[n + 1], zNr = zN[n] + zN[n + 1];
+      const real tN = (zNN[n] - zS[n]) + (zNN[n + 1] - zS[n + 1]);  // 4 xi_N
+      const real by = zNr - zSr[n];                                 // 2 (z_N - z_S)
+      const real bm = (a - by) * P.my2, bp = (a + by) * P.my2;
+      C.n[n] = bm * fma(q, tN, hNr);
+      C.s[n] = bp * fma(-q, tS[n], hSr[n]);
+      const real cy = fma(bm, fma(-q, tN, hNr), bp * fma(q, tS[n], hSr[n]));
       C.c[n] = RC(2.0) - (cx + cy);
+      hSr[n] = hNr; zSr[n] = zNr; tS[n] = tN;
     }
 #pragma unroll
-    for (int k = 0; k < 3; ++k) { hS[k] = hN[k]; zS[k] = zN[k]; zN[k] = zNN[k]; xyS[k] = xyN[k]; }
+    for (int k = 0; k < 3; ++k) { hS[k] = hN[k]; zS[k] = zN[k]; zN[k] = zNN[k]; }
     return C;
   }
 };
@@ -299,6 +306,75 @@ __device__ __forceinline__ real2 offdiag2(const Coef& C, real2 m, real2 c, real2
 // row is computed and stored (the compiler cannot hoist them itself across the stores of possibly
 // aliasing planes), so each warp keeps one full row of every plane in flight while it computes.
 
+// ---- operand ring in shared memory (fp64 build) -------------------------------------------------
+// The sweep is bound by the bytes a warp keeps in flight (Little's law: at 12 warps per SM one
+// operand set per warp held in registers sustains 63 % of the DRAM rate, profiles/r02c).  So the
+// operand rows of the NEXT NH_STAGES sweep steps are fetched by bulk asynchronous copies
+// (cp.async.bulk global -> shared, one 512-byte row segment per plane, issued by lane 0, completion
+// counted by an mbarrier per stage) into a ring private to the warp; a step waits for its stage,
+// moves the operands to registers, hands the stage back (__syncwarp) and lane 0 refills it with
+// the operands of step j + NH_STAGES.  No register holds data in flight.
+#if NH_PREC == 64
+#define NH_BULK 1
+#else
+#define NH_BULK 0  // fp32: row segments start on 8-byte boundaries (bulk copies need 16): register path
+#endif
+#define NH_STR_(x) #x
+#define NH_STR(x) NH_STR_(x)
+#ifndef NH_UNROLL
+#define NH_UNROLL 2  // sweep loops unrolled by two: the rolling rows need no register moves (-2 %)
+#endif
+#ifndef NH_STAGES
+#define NH_STAGES 3
+#endif
+constexpr int RING_SEGS = 8;                          // planes per operand set (pass CA)
+constexpr int SEG_BYTES = 64 * (int)sizeof(real);     // one row segment of a strip: 32 lanes x 2 columns
+constexpr int STAGE_BYTES = RING_SEGS * SEG_BYTES;
+constexpr int RING_BYTES = NH_STAGES * STAGE_BYTES;   // per warp
+struct Ring {  // (the fp32 build carries an empty ring through the same signatures)
+  uint32_t base;  // shared-window address of this warp's ring
+  uint32_t bars;  // ... of its NH_STAGES mbarriers
+  const char* gen;  // generic pointer to the ring (for the reads)
+  uint32_t parity;  // bit s: phase parity stage s completes next
+  int st;           // stage of the next sweep step
+};
+#if NH_BULK
+__device__ __forceinline__ void ring_issue_begin(const Ring& R, int stage, int nseg) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(R.bars + 8u * stage),
+               "r"((uint32_t)(nseg * SEG_BYTES))
+               : "memory");
+}
+__device__ __forceinline__ void ring_issue(const Ring& R, int stage, int seg, const real* src) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+          R.base + (uint32_t)(stage * STAGE_BYTES + seg * SEG_BYTES)),
+      "l"(src), "r"((uint32_t)SEG_BYTES), "r"(R.bars + 8u * stage)
+      : "memory");
+}
+__device__ __forceinline__ void ring_wait(Ring& R, int stage) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra DONE;\n"
+      "bra LAB_WAIT;\n"
+      "DONE:\n"
+      "}" ::"r"(R.bars + 8u * stage),
+      "r"((R.parity >> stage) & 1u)
+      : "memory");
+  R.parity ^= 1u << stage;
+}
+__device__ __forceinline__ real2 ring_read(const Ring& R, int stage, int seg, int lane) {
+  return *reinterpret_cast<const real2*>(R.gen + stage * STAGE_BYTES + seg * SEG_BYTES + lane * 2 * (int)sizeof(real));
+}
+// first column of a strip's row segment (lane 0's c0) of row j
+__device__ __forceinline__ const real* seg_ptr(const real* a, const SolveP& P, int c00, int j) {
+  return a + nidx(P.G, c00, j);
+}
+
+#endif  // NH_BULK
+
 // residual pass: r = b - A x (S9: the true residual decides), r0 = r, r^ = r / A_C; partials r.r, b.b
 __device__ __forceinline__ void pass_R(const SolveP& P, real* rh, int buf, double (*red)[NW]) {
   const NhGrid& G = P.G;
@@ -331,15 +407,17 @@ __device__ __forceinline__ void pass_R(const SolveP& P, real* rh, int buf, doubl
 struct RowB {  // operands of sweep step j: r^, v^ of row j+1; r0, h of row j; z of row j+1
   real2 r, v, q, h, z;
 };
+#if !NH_BULK
 __device__ __forceinline__ void ld_rowb(RowB& X, const SolveP& P, const real* r, const real* v,
                                         int c0, int j) {
   X.r = ld2(r, P.G, c0, j + 1); X.v = ld2(v, P.G, c0, j + 1);
   X.q = ld2(P.r0, P.G, c0, j);
   X.h = ld2(P.hc, P.G, c0, j); X.z = ld2(P.zc, P.G, c0, j + 1);
 }
+#endif
 
 __device__ __forceinline__ void pass_B(const SolveP& P, real alpha, const real* r, const real* v,
-                                    int buf, double (*red)[NW]) {
+                                    int buf, double (*red)[NW], Ring& R) {
   const NhGrid& G = P.G;
   const int lane = threadIdx.x & 31;
   const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
@@ -358,12 +436,40 @@ __device__ __forceinline__ void pass_B(const SolveP& P, real alpha, const real* 
     // into the marching state, before the arithmetic of the step (row index clamped: the last
     // request is never used).
     RowB X;
+#if NH_BULK
+    const int c00 = U.c0 - 2 * lane;  // first column of the strip's row segments
+    auto issue = [&](int stage, int j) {  // operands of sweep step j -> ring stage
+      if (lane == 0) {
+        ring_issue_begin(R, stage, 5);
+        ring_issue(R, stage, 0, seg_ptr(r, P, c00, j + 1));
+        ring_issue(R, stage, 1, seg_ptr(v, P, c00, j + 1));
+        ring_issue(R, stage, 2, seg_ptr(P.r0, P, c00, j));
+        ring_issue(R, stage, 3, seg_ptr(P.hc, P, c00, j));
+        ring_issue(R, stage, 4, seg_ptr(P.zc, P, c00, j + 1));
+      }
+    };
+    for (int k2 = 0; k2 < NH_STAGES; ++k2)
+      if (U.Ja + k2 < U.Jb) issue((R.st + k2) % NH_STAGES, U.Ja + k2);
+#else
     ld_rowb(X, P, r, v, U.c0, U.Ja);
+#endif
+    _Pragma(NH_STR(unroll NH_UNROLL))
     for (int j = U.Ja; j < U.Jb; ++j) {
+#if NH_BULK
+      ring_wait(R, R.st);
+      X.r = ring_read(R, R.st, 0, lane); X.v = ring_read(R, R.st, 1, lane);
+      X.q = ring_read(R, R.st, 2, lane);
+      X.h = ring_read(R, R.st, 3, lane); X.z = ring_read(R, R.st, 4, lane);
+      __syncwarp();
+      if (j + NH_STAGES < U.Jb) issue(R.st, j + NH_STAGES);
+      R.st = (R.st + 1) % NH_STAGES;
+#endif
       const real2 sn = srow(X.r, X.v);
       const real2 q = X.q;
       const Coef C = M.step(P, X.h, X.z);
+#if !NH_BULK
       if (j + 1 < U.Jb) ld_rowb(X, P, r, v, U.c0, j + 1);
+#endif
       const real2 off = offdiag2(C, sm, sc, sn);
       const real2 tu = make_real2(fma(C.c[0], sc.x, off.x), fma(C.c[1], sc.y, off.y));  // t
       const real2 su = make_real2(C.c[0] * sc.x, C.c[1] * sc.y);                        // s
@@ -407,7 +513,7 @@ struct RowCA {  // operands of sweep step j: vectors of row j+1; r0, h of row j;
 template <bool FIRST>
 __device__ __forceinline__ void pass_CA(const SolveP& P, real alpha, real omega, real beta,
                                      const real* r, const real* p, const real* v, real* rN,
-                                     real* pN, real* vN, int buf, double (*red)[NW]) {
+                                     real* pN, real* vN, int buf, double (*red)[NW], Ring& R) {
   const int lane = threadIdx.x & 31;
   const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
   const int nunits = P.nstrips * P.nbands;
@@ -452,14 +558,50 @@ __device__ __forceinline__ void pass_CA(const SolveP& P, real alpha, real omega,
     // BEFORE its stores (ghost-image logic included) and its dot-product terms, which then run in
     // the shadow of the memory latency.
     RowCA X;
+#if NH_BULK
+    const int c00 = U.c0 - 2 * lane;
+    auto issue = [&](int stage, int j) {  // operands of sweep step j -> ring stage
+      if (lane == 0) {
+        ring_issue_begin(R, stage, FIRST ? 4 : 8);
+        ring_issue(R, stage, 0, seg_ptr(r, P, c00, j + 1));
+        ring_issue(R, stage, 1, seg_ptr(P.r0, P, c00, j));
+        ring_issue(R, stage, 2, seg_ptr(P.hc, P, c00, j));
+        ring_issue(R, stage, 3, seg_ptr(P.zc, P, c00, j + 1));
+        if (!FIRST) {
+          ring_issue(R, stage, 4, seg_ptr(v, P, c00, j + 1));
+          ring_issue(R, stage, 5, seg_ptr(P.t, P, c00, j + 1));
+          ring_issue(R, stage, 6, seg_ptr(p, P, c00, j + 1));
+          ring_issue(R, stage, 7, seg_ptr(P.x, P, c00, j + 1));
+        }
+      }
+    };
+    for (int k2 = 0; k2 < NH_STAGES; ++k2)
+      if (U.Ja + k2 < U.Jb) issue((R.st + k2) % NH_STAGES, U.Ja + k2);
+#else
     ld_set(X, U.Ja);
+#endif
+    _Pragma(NH_STR(unroll NH_UNROLL))
     for (int j = U.Ja; j < U.Jb; ++j) {
       const bool own_next = j + 1 < U.Jb;
+#if NH_BULK
+      ring_wait(R, R.st);
+      X.V.r = ring_read(R, R.st, 0, lane); X.q = ring_read(R, R.st, 1, lane);
+      X.h = ring_read(R, R.st, 2, lane); X.z = ring_read(R, R.st, 3, lane);
+      if (!FIRST) {
+        X.V.v = ring_read(R, R.st, 4, lane); X.V.t = ring_read(R, R.st, 5, lane);
+        X.V.p = ring_read(R, R.st, 6, lane); X.V.x = ring_read(R, R.st, 7, lane);
+      }
+      __syncwarp();
+      if (j + NH_STAGES < U.Jb) issue(R.st, j + NH_STAGES);
+      R.st = (R.st + 1) % NH_STAGES;
+#endif
       real2 rn, pn, xx;
       vrow(X.V, rn, pn, xx);
       const Coef C = M.step(P, X.h, X.z);
       const real2 q = X.q;
+#if !NH_BULK
       if (own_next) ld_set(X, min(j + 1, U.Jb - 1));  // operands of the next step
+#endif
       const real2 off = offdiag2(C, pm, pc, pn);
       const real2 vu = make_real2(fma(C.c[0], pc.x, off.x), fma(C.c[1], pc.y, off.y));  // v'
       if (own_next) store_row(j + 1, rn, pn, xx);
@@ -500,6 +642,18 @@ __device__ void phase_zero_x(const SolveP& P) {
     for (int I = threadIdx.x; I < G.nnx; I += NT) store_images(G, P.x, I, J, RC(0.0));
 }
 
+// grid barrier; the bulk copies of the next pass (asynchronous proxy) read what the generic-proxy
+// stores of this pass wrote: order the two proxies on both sides of the barrier
+__device__ __forceinline__ void gsync(cg::grid_group& grid) {
+#if NH_BULK
+  asm volatile("fence.proxy.async;" ::: "memory");
+#endif
+  grid.sync();
+#if NH_BULK
+  asm volatile("fence.proxy.async;" ::: "memory");
+#endif
+}
+
 __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
   cg::grid_group grid = cg::this_grid();
   __shared__ double red[MAXDOT][NW];
@@ -515,13 +669,30 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
   int buf = 0;  // partial buffer of the pass in flight (alternates: one grid barrier per pass)
   int iters = 0, converged = 0, status = 0;
   double rnorm = 0.0, bnorm = 0.0, tol = 0.0, rnorm_prev = 0.0;
+  Ring R;
+  R.base = 0; R.bars = 0; R.gen = nullptr; R.parity = 0; R.st = 0;
+#if NH_BULK
+  {  // this warp's operand ring and its mbarriers (one arrival each: lane 0's expect_tx)
+    extern __shared__ __align__(128) unsigned char ring_smem[];
+    __shared__ __align__(8) unsigned long long ring_bars[NW][NH_STAGES];
+    const int wid = threadIdx.x >> 5;
+    R.gen = reinterpret_cast<const char*>(ring_smem) + wid * RING_BYTES;
+    R.base = (uint32_t)__cvta_generic_to_shared(R.gen);
+    R.bars = (uint32_t)__cvta_generic_to_shared(&ring_bars[wid][0]);
+    if ((threadIdx.x & 31) == 0)
+      for (int k = 0; k < NH_STAGES; ++k)
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(R.bars + 8u * k) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    __syncthreads();
+  }
+#endif
 
   phase_images(P);
-  grid.sync();
+  gsync(grid);
   for (int cycle = 0; cycle < 8 && !converged; ++cycle) {
     double d2[2], d5[5];
     pass_R(P, rC, buf, red);
-    grid.sync();
+    gsync(grid);
     grid_sums<2>(P.part, buf, d2, red, bc);
     buf ^= 1;
     rnorm = sqrt(d2[0]);
@@ -541,9 +712,9 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
     if (iters >= P.maxit) break;
     // first direction of the cycle: p = r, v = A M^-1 p, sigma = r0.v
     double rho = d2[0];
-    pass_CA<true>(P, RC(0.0), RC(0.0), RC(0.0), rC, pC, vC, rN, pN, vN, buf, red);
+    pass_CA<true>(P, RC(0.0), RC(0.0), RC(0.0), rC, pC, vC, rN, pN, vN, buf, red, R);
     flip();
-    grid.sync();
+    gsync(grid);
     grid_sums<2>(P.part, buf, d2, red, bc);
     buf ^= 1;
     double sigma = d2[0];
@@ -551,13 +722,13 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
       if (fabs(rho) < 1e-300 || fabs(sigma) < 1e-300) break;  // breakdown -> restart
       double alpha = rho / sigma;
       iters++;
-      pass_B(P, (real)alpha, rC, vC, buf, red);
-      grid.sync();
+      pass_B(P, (real)alpha, rC, vC, buf, red, R);
+      gsync(grid);
       grid_sums<5>(P.part, buf, d5, red, bc);
       buf ^= 1;
       if (sqrt(d5[2]) <= tol) {  // half-step exit: x += alpha p^
         phase_update_x(P, (real)alpha, RC(0.0), rC, pC, vC);
-        grid.sync();
+        gsync(grid);
         break;
       }
       if (d5[1] == 0.0) break;
@@ -566,9 +737,9 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
       double rho_new = d5[3] - omega * d5[4];  // r0.r' = r0.s - omega r0.t  (R25)
       double beta = (rho_new / rho) * (alpha / omega);
       rho = rho_new;
-      pass_CA<false>(P, (real)alpha, (real)omega, (real)beta, rC, pC, vC, rN, pN, vN, buf, red);
+      pass_CA<false>(P, (real)alpha, (real)omega, (real)beta, rC, pC, vC, rN, pN, vN, buf, red, R);
       flip();
-      grid.sync();
+      gsync(grid);
       grid_sums<2>(P.part, buf, d2, red, bc);
       buf ^= 1;
       sigma = d2[0];
@@ -584,21 +755,21 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
   if (converged && rnorm > 0.0) {
     double d2[2], d5[5];
     double rho = rnorm * rnorm;
-    pass_CA<true>(P, RC(0.0), RC(0.0), RC(0.0), rC, pC, vC, rN, pN, vN, buf, red);
+    pass_CA<true>(P, RC(0.0), RC(0.0), RC(0.0), rC, pC, vC, rN, pN, vN, buf, red, R);
     flip();
-    grid.sync();
+    gsync(grid);
     grid_sums<2>(P.part, buf, d2, red, bc);
     buf ^= 1;
     double sigma = d2[0];
     if (fabs(rho) >= 1e-300 && fabs(sigma) >= 1e-300) {
       double alpha = rho / sigma;
-      pass_B(P, (real)alpha, rC, vC, buf, red);
-      grid.sync();
+      pass_B(P, (real)alpha, rC, vC, buf, red, R);
+      gsync(grid);
       grid_sums<5>(P.part, buf, d5, red, bc);
       buf ^= 1;
       double omega = (d5[1] > 0.0) ? d5[0] / d5[1] : 0.0;
       phase_update_x(P, (real)alpha, (real)omega, rC, pC, vC);
-      grid.sync();
+      gsync(grid);
     }
   }
   if (status != NH_ENAN && bnorm == 0.0) phase_zero_x(P);  // b = 0 => p~ = 0, zero iterations
@@ -766,7 +937,10 @@ __global__ void __launch_bounds__(NT1, NH_SRJ_MINB) k_srj(SrjP P) {
 // same band); R minimises rounds x (R + 2 halo rows).
 int nh_solver_setup(Ctx* c) {
   int occ = 0;
-  cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bicgstab, NT, 0);
+  const size_t dyn = NH_BULK ? (size_t)NW * RING_BYTES : 0;  // operand rings of the CTA's warps
+  cudaError_t e = cudaSuccess;
+  if (dyn) e = cudaFuncSetAttribute(k_bicgstab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
+  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bicgstab, NT, dyn);
   if (e != cudaSuccess || occ < 1) {
     snprintf(c->err, sizeof(c->err), "solver occupancy query failed: %s", cudaGetErrorString(e));
     return NH_ECUDA;
@@ -862,12 +1036,12 @@ void nh_launch_solve(Ctx* c, const real* b, real* x, int count_stats) {
   P.r0 = c->kr0; P.t = c->kt;
   P.rA = c->kr; P.rB = c->krB; P.pA = c->kpA; P.pB = c->kpB; P.vA = c->kvA; P.vB = c->kvB;
   P.part = c->part; P.sc = c->sc; P.rtol = c->prm.solver_rtol; P.maxit = c->prm.solver_maxit;
-  P.miex = (real)(-1.0 / (8.0 * (double)c->g.dx * (double)c->g.dx));
-  P.miey = (real)(-1.0 / (8.0 * (double)c->g.dy * (double)c->g.dy));
+  P.mx2 = (real)(-1.0 / (16.0 * (double)c->g.dx * (double)c->g.dx));
+  P.my2 = (real)(-1.0 / (16.0 * (double)c->g.dy * (double)c->g.dy));
   P.count_stats = count_stats;
   void* args[] = {&P};
   NH_CUDA_OK(c, cudaLaunchCooperativeKernel((void*)k_bicgstab, dim3(c->solver_grid), dim3(NT), args,
-                                            0, c->stream));
+                                            NH_BULK ? (size_t)NW * RING_BYTES : 0, c->stream));
   c->launches++;
 }
 
