@@ -67,9 +67,10 @@ constexpr int NT = NH_NT, NW = NT / 32;  // CTA size, warps per CTA
 constexpr int SW = 60;                 // owned columns per warp strip
 constexpr int MAXDOT = 5;
 // small grids: at least this many rows per warp before CTAs are added (a warp marches its rows one
-// memory latency at a time; measured at 512 x 8 ... 512^2: 8 rows 18-20 us per iteration, 4 rows 13-15)
+// memory latency at a time; us per iteration at 512 x 8 / 256^2 / 512^2: 4 rows 13.8 / 14.3 / 17.4,
+// 2 rows 10.5 / 11.9 / 15.6, 1 row 8.5 / 11.3 / 15.6; no effect from 1024^2 up)
 #ifndef NH_MINROWS
-#define NH_MINROWS 4
+#define NH_MINROWS 1
 #endif
 
 struct SolveP {
@@ -306,74 +307,11 @@ __device__ __forceinline__ real2 offdiag2(const Coef& C, real2 m, real2 c, real2
 // row is computed and stored (the compiler cannot hoist them itself across the stores of possibly
 // aliasing planes), so each warp keeps one full row of every plane in flight while it computes.
 
-// ---- operand ring in shared memory (fp64 build) -------------------------------------------------
-// The sweep is bound by the bytes a warp keeps in flight (Little's law: at 12 warps per SM one
-// operand set per warp held in registers sustains 63 % of the DRAM rate, profiles/r02c).  So the
-// operand rows of the NEXT NH_STAGES sweep steps are fetched by bulk asynchronous copies
-// (cp.async.bulk global -> shared, one 512-byte row segment per plane, issued by lane 0, completion
-// counted by an mbarrier per stage) into a ring private to the warp; a step waits for its stage,
-// moves the operands to registers, hands the stage back (__syncwarp) and lane 0 refills it with
-// the operands of step j + NH_STAGES.  No register holds data in flight.
-#if NH_PREC == 64
-#define NH_BULK 1
-#else
-#define NH_BULK 0  // fp32: row segments start on 8-byte boundaries (bulk copies need 16): register path
-#endif
 #define NH_STR_(x) #x
 #define NH_STR(x) NH_STR_(x)
 #ifndef NH_UNROLL
 #define NH_UNROLL 2  // sweep loops unrolled by two: the rolling rows need no register moves (-2 %)
 #endif
-#ifndef NH_STAGES
-#define NH_STAGES 3
-#endif
-constexpr int RING_SEGS = 8;                          // planes per operand set (pass CA)
-constexpr int SEG_BYTES = 64 * (int)sizeof(real);     // one row segment of a strip: 32 lanes x 2 columns
-constexpr int STAGE_BYTES = RING_SEGS * SEG_BYTES;
-constexpr int RING_BYTES = NH_STAGES * STAGE_BYTES;   // per warp
-struct Ring {  // (the fp32 build carries an empty ring through the same signatures)
-  uint32_t base;  // shared-window address of this warp's ring
-  uint32_t bars;  // ... of its NH_STAGES mbarriers
-  const char* gen;  // generic pointer to the ring (for the reads)
-  uint32_t parity;  // bit s: phase parity stage s completes next
-  int st;           // stage of the next sweep step
-};
-#if NH_BULK
-__device__ __forceinline__ void ring_issue_begin(const Ring& R, int stage, int nseg) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(R.bars + 8u * stage),
-               "r"((uint32_t)(nseg * SEG_BYTES))
-               : "memory");
-}
-__device__ __forceinline__ void ring_issue(const Ring& R, int stage, int seg, const real* src) {
-  asm volatile(
-      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-          R.base + (uint32_t)(stage * STAGE_BYTES + seg * SEG_BYTES)),
-      "l"(src), "r"((uint32_t)SEG_BYTES), "r"(R.bars + 8u * stage)
-      : "memory");
-}
-__device__ __forceinline__ void ring_wait(Ring& R, int stage) {
-  asm volatile(
-      "{\n"
-      ".reg .pred P1;\n"
-      "LAB_WAIT:\n"
-      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
-      "@P1 bra DONE;\n"
-      "bra LAB_WAIT;\n"
-      "DONE:\n"
-      "}" ::"r"(R.bars + 8u * stage),
-      "r"((R.parity >> stage) & 1u)
-      : "memory");
-  R.parity ^= 1u << stage;
-}
-__device__ __forceinline__ real2 ring_read(const Ring& R, int stage, int seg, int lane) {
-  return *reinterpret_cast<const real2*>(R.gen + stage * STAGE_BYTES + seg * SEG_BYTES + lane * 2 * (int)sizeof(real));
-}
-// first column of a strip's row segment (lane 0's c0) of row j
-__device__ __forceinline__ const real* seg_ptr(const real* a, const SolveP& P, int c00, int j) {
-  return a + nidx(P.G, c00, j);
-}
-
-#endif  // NH_BULK
 
 // residual pass: r = b - A x (S9: the true residual decides), r0 = r, r^ = r / A_C; partials r.r, b.b
 __device__ __forceinline__ void pass_R(const SolveP& P, real* rh, int buf, double (*red)[NW]) {
@@ -407,17 +345,15 @@ __device__ __forceinline__ void pass_R(const SolveP& P, real* rh, int buf, doubl
 struct RowB {  // operands of sweep step j: r^, v^ of row j+1; r0, h of row j; z of row j+1
   real2 r, v, q, h, z;
 };
-#if !NH_BULK
 __device__ __forceinline__ void ld_rowb(RowB& X, const SolveP& P, const real* r, const real* v,
                                         int c0, int j) {
   X.r = ld2(r, P.G, c0, j + 1); X.v = ld2(v, P.G, c0, j + 1);
   X.q = ld2(P.r0, P.G, c0, j);
   X.h = ld2(P.hc, P.G, c0, j); X.z = ld2(P.zc, P.G, c0, j + 1);
 }
-#endif
 
 __device__ __forceinline__ void pass_B(const SolveP& P, real alpha, const real* r, const real* v,
-                                    int buf, double (*red)[NW], Ring& R) {
+                                    int buf, double (*red)[NW]) {
   const NhGrid& G = P.G;
   const int lane = threadIdx.x & 31;
   const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
@@ -436,40 +372,13 @@ __device__ __forceinline__ void pass_B(const SolveP& P, real alpha, const real* 
     // into the marching state, before the arithmetic of the step (row index clamped: the last
     // request is never used).
     RowB X;
-#if NH_BULK
-    const int c00 = U.c0 - 2 * lane;  // first column of the strip's row segments
-    auto issue = [&](int stage, int j) {  // operands of sweep step j -> ring stage
-      if (lane == 0) {
-        ring_issue_begin(R, stage, 5);
-        ring_issue(R, stage, 0, seg_ptr(r, P, c00, j + 1));
-        ring_issue(R, stage, 1, seg_ptr(v, P, c00, j + 1));
-        ring_issue(R, stage, 2, seg_ptr(P.r0, P, c00, j));
-        ring_issue(R, stage, 3, seg_ptr(P.hc, P, c00, j));
-        ring_issue(R, stage, 4, seg_ptr(P.zc, P, c00, j + 1));
-      }
-    };
-    for (int k2 = 0; k2 < NH_STAGES; ++k2)
-      if (U.Ja + k2 < U.Jb) issue((R.st + k2) % NH_STAGES, U.Ja + k2);
-#else
     ld_rowb(X, P, r, v, U.c0, U.Ja);
-#endif
     _Pragma(NH_STR(unroll NH_UNROLL))
     for (int j = U.Ja; j < U.Jb; ++j) {
-#if NH_BULK
-      ring_wait(R, R.st);
-      X.r = ring_read(R, R.st, 0, lane); X.v = ring_read(R, R.st, 1, lane);
-      X.q = ring_read(R, R.st, 2, lane);
-      X.h = ring_read(R, R.st, 3, lane); X.z = ring_read(R, R.st, 4, lane);
-      __syncwarp();
-      if (j + NH_STAGES < U.Jb) issue(R.st, j + NH_STAGES);
-      R.st = (R.st + 1) % NH_STAGES;
-#endif
       const real2 sn = srow(X.r, X.v);
       const real2 q = X.q;
       const Coef C = M.step(P, X.h, X.z);
-#if !NH_BULK
       if (j + 1 < U.Jb) ld_rowb(X, P, r, v, U.c0, j + 1);
-#endif
       const real2 off = offdiag2(C, sm, sc, sn);
       const real2 tu = make_real2(fma(C.c[0], sc.x, off.x), fma(C.c[1], sc.y, off.y));  // t
       const real2 su = make_real2(C.c[0] * sc.x, C.c[1] * sc.y);                        // s
@@ -513,7 +422,7 @@ struct RowCA {  // operands of sweep step j: vectors of row j+1; r0, h of row j;
 template <bool FIRST>
 __device__ __forceinline__ void pass_CA(const SolveP& P, real alpha, real omega, real beta,
                                      const real* r, const real* p, const real* v, real* rN,
-                                     real* pN, real* vN, int buf, double (*red)[NW], Ring& R) {
+                                     real* pN, real* vN, int buf, double (*red)[NW]) {
   const int lane = threadIdx.x & 31;
   const int gw = blockIdx.x * NW + (threadIdx.x >> 5), tw = gridDim.x * NW;
   const int nunits = P.nstrips * P.nbands;
@@ -558,50 +467,15 @@ __device__ __forceinline__ void pass_CA(const SolveP& P, real alpha, real omega,
     // BEFORE its stores (ghost-image logic included) and its dot-product terms, which then run in
     // the shadow of the memory latency.
     RowCA X;
-#if NH_BULK
-    const int c00 = U.c0 - 2 * lane;
-    auto issue = [&](int stage, int j) {  // operands of sweep step j -> ring stage
-      if (lane == 0) {
-        ring_issue_begin(R, stage, FIRST ? 4 : 8);
-        ring_issue(R, stage, 0, seg_ptr(r, P, c00, j + 1));
-        ring_issue(R, stage, 1, seg_ptr(P.r0, P, c00, j));
-        ring_issue(R, stage, 2, seg_ptr(P.hc, P, c00, j));
-        ring_issue(R, stage, 3, seg_ptr(P.zc, P, c00, j + 1));
-        if (!FIRST) {
-          ring_issue(R, stage, 4, seg_ptr(v, P, c00, j + 1));
-          ring_issue(R, stage, 5, seg_ptr(P.t, P, c00, j + 1));
-          ring_issue(R, stage, 6, seg_ptr(p, P, c00, j + 1));
-          ring_issue(R, stage, 7, seg_ptr(P.x, P, c00, j + 1));
-        }
-      }
-    };
-    for (int k2 = 0; k2 < NH_STAGES; ++k2)
-      if (U.Ja + k2 < U.Jb) issue((R.st + k2) % NH_STAGES, U.Ja + k2);
-#else
     ld_set(X, U.Ja);
-#endif
     _Pragma(NH_STR(unroll NH_UNROLL))
     for (int j = U.Ja; j < U.Jb; ++j) {
       const bool own_next = j + 1 < U.Jb;
-#if NH_BULK
-      ring_wait(R, R.st);
-      X.V.r = ring_read(R, R.st, 0, lane); X.q = ring_read(R, R.st, 1, lane);
-      X.h = ring_read(R, R.st, 2, lane); X.z = ring_read(R, R.st, 3, lane);
-      if (!FIRST) {
-        X.V.v = ring_read(R, R.st, 4, lane); X.V.t = ring_read(R, R.st, 5, lane);
-        X.V.p = ring_read(R, R.st, 6, lane); X.V.x = ring_read(R, R.st, 7, lane);
-      }
-      __syncwarp();
-      if (j + NH_STAGES < U.Jb) issue(R.st, j + NH_STAGES);
-      R.st = (R.st + 1) % NH_STAGES;
-#endif
       real2 rn, pn, xx;
       vrow(X.V, rn, pn, xx);
       const Coef C = M.step(P, X.h, X.z);
       const real2 q = X.q;
-#if !NH_BULK
       if (own_next) ld_set(X, min(j + 1, U.Jb - 1));  // operands of the next step
-#endif
       const real2 off = offdiag2(C, pm, pc, pn);
       const real2 vu = make_real2(fma(C.c[0], pc.x, off.x), fma(C.c[1], pc.y, off.y));  // v'
       if (own_next) store_row(j + 1, rn, pn, xx);
@@ -642,18 +516,6 @@ __device__ void phase_zero_x(const SolveP& P) {
     for (int I = threadIdx.x; I < G.nnx; I += NT) store_images(G, P.x, I, J, RC(0.0));
 }
 
-// grid barrier; the bulk copies of the next pass (asynchronous proxy) read what the generic-proxy
-// stores of this pass wrote: order the two proxies on both sides of the barrier
-__device__ __forceinline__ void gsync(cg::grid_group& grid) {
-#if NH_BULK
-  asm volatile("fence.proxy.async;" ::: "memory");
-#endif
-  grid.sync();
-#if NH_BULK
-  asm volatile("fence.proxy.async;" ::: "memory");
-#endif
-}
-
 __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
   cg::grid_group grid = cg::this_grid();
   __shared__ double red[MAXDOT][NW];
@@ -669,30 +531,13 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
   int buf = 0;  // partial buffer of the pass in flight (alternates: one grid barrier per pass)
   int iters = 0, converged = 0, status = 0;
   double rnorm = 0.0, bnorm = 0.0, tol = 0.0, rnorm_prev = 0.0;
-  Ring R;
-  R.base = 0; R.bars = 0; R.gen = nullptr; R.parity = 0; R.st = 0;
-#if NH_BULK
-  {  // this warp's operand ring and its mbarriers (one arrival each: lane 0's expect_tx)
-    extern __shared__ __align__(128) unsigned char ring_smem[];
-    __shared__ __align__(8) unsigned long long ring_bars[NW][NH_STAGES];
-    const int wid = threadIdx.x >> 5;
-    R.gen = reinterpret_cast<const char*>(ring_smem) + wid * RING_BYTES;
-    R.base = (uint32_t)__cvta_generic_to_shared(R.gen);
-    R.bars = (uint32_t)__cvta_generic_to_shared(&ring_bars[wid][0]);
-    if ((threadIdx.x & 31) == 0)
-      for (int k = 0; k < NH_STAGES; ++k)
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(R.bars + 8u * k) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    __syncthreads();
-  }
-#endif
 
   phase_images(P);
-  gsync(grid);
+  grid.sync();
   for (int cycle = 0; cycle < 8 && !converged; ++cycle) {
     double d2[2], d5[5];
     pass_R(P, rC, buf, red);
-    gsync(grid);
+    grid.sync();
     grid_sums<2>(P.part, buf, d2, red, bc);
     buf ^= 1;
     rnorm = sqrt(d2[0]);
@@ -712,9 +557,9 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
     if (iters >= P.maxit) break;
     // first direction of the cycle: p = r, v = A M^-1 p, sigma = r0.v
     double rho = d2[0];
-    pass_CA<true>(P, RC(0.0), RC(0.0), RC(0.0), rC, pC, vC, rN, pN, vN, buf, red, R);
+    pass_CA<true>(P, RC(0.0), RC(0.0), RC(0.0), rC, pC, vC, rN, pN, vN, buf, red);
     flip();
-    gsync(grid);
+    grid.sync();
     grid_sums<2>(P.part, buf, d2, red, bc);
     buf ^= 1;
     double sigma = d2[0];
@@ -722,13 +567,13 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
       if (fabs(rho) < 1e-300 || fabs(sigma) < 1e-300) break;  // breakdown -> restart
       double alpha = rho / sigma;
       iters++;
-      pass_B(P, (real)alpha, rC, vC, buf, red, R);
-      gsync(grid);
+      pass_B(P, (real)alpha, rC, vC, buf, red);
+      grid.sync();
       grid_sums<5>(P.part, buf, d5, red, bc);
       buf ^= 1;
       if (sqrt(d5[2]) <= tol) {  // half-step exit: x += alpha p^
         phase_update_x(P, (real)alpha, RC(0.0), rC, pC, vC);
-        gsync(grid);
+        grid.sync();
         break;
       }
       if (d5[1] == 0.0) break;
@@ -737,9 +582,9 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
       double rho_new = d5[3] - omega * d5[4];  // r0.r' = r0.s - omega r0.t  (R25)
       double beta = (rho_new / rho) * (alpha / omega);
       rho = rho_new;
-      pass_CA<false>(P, (real)alpha, (real)omega, (real)beta, rC, pC, vC, rN, pN, vN, buf, red, R);
+      pass_CA<false>(P, (real)alpha, (real)omega, (real)beta, rC, pC, vC, rN, pN, vN, buf, red);
       flip();
-      gsync(grid);
+      grid.sync();
       grid_sums<2>(P.part, buf, d2, red, bc);
       buf ^= 1;
       sigma = d2[0];
@@ -755,21 +600,21 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
   if (converged && rnorm > 0.0) {
     double d2[2], d5[5];
     double rho = rnorm * rnorm;
-    pass_CA<true>(P, RC(0.0), RC(0.0), RC(0.0), rC, pC, vC, rN, pN, vN, buf, red, R);
+    pass_CA<true>(P, RC(0.0), RC(0.0), RC(0.0), rC, pC, vC, rN, pN, vN, buf, red);
     flip();
-    gsync(grid);
+    grid.sync();
     grid_sums<2>(P.part, buf, d2, red, bc);
     buf ^= 1;
     double sigma = d2[0];
     if (fabs(rho) >= 1e-300 && fabs(sigma) >= 1e-300) {
       double alpha = rho / sigma;
-      pass_B(P, (real)alpha, rC, vC, buf, red, R);
-      gsync(grid);
+      pass_B(P, (real)alpha, rC, vC, buf, red);
+      grid.sync();
       grid_sums<5>(P.part, buf, d5, red, bc);
       buf ^= 1;
       double omega = (d5[1] > 0.0) ? d5[0] / d5[1] : 0.0;
       phase_update_x(P, (real)alpha, (real)omega, rC, pC, vC);
-      gsync(grid);
+      grid.sync();
     }
   }
   if (status != NH_ENAN && bnorm == 0.0) phase_zero_x(P);  // b = 0 => p~ = 0, zero iterations
@@ -937,10 +782,7 @@ __global__ void __launch_bounds__(NT1, NH_SRJ_MINB) k_srj(SrjP P) {
 // same band); R minimises rounds x (R + 2 halo rows).
 int nh_solver_setup(Ctx* c) {
   int occ = 0;
-  const size_t dyn = NH_BULK ? (size_t)NW * RING_BYTES : 0;  // operand rings of the CTA's warps
-  cudaError_t e = cudaSuccess;
-  if (dyn) e = cudaFuncSetAttribute(k_bicgstab, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn);
-  if (e == cudaSuccess) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bicgstab, NT, dyn);
+  cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_bicgstab, NT, 0);
   if (e != cudaSuccess || occ < 1) {
     snprintf(c->err, sizeof(c->err), "solver occupancy query failed: %s", cudaGetErrorString(e));
     return NH_ECUDA;
@@ -954,13 +796,13 @@ int nh_solver_setup(Ctx* c) {
   const long long tw = grid * NW;
   int bestR = nny;
   long long best = -1;
-  for (int R = 4; R <= nny; ++R) {
+  for (int R = NH_MINROWS; R <= nny; ++R) {
     long long nb = (nny + R - 1) / R;
     long long rounds = (nstrips * nb + tw - 1) / tw;
     long long cost = rounds * (R + 2);
     if (best < 0 || cost < best) { best = cost; bestR = R; }
   }
-  if (nny < 4) bestR = nny;
+  if (nny < NH_MINROWS) bestR = nny;
   c->solver_occ = occ;
   c->solver_grid = (int)grid;
   c->solver_nstrips = nstrips;
@@ -985,13 +827,13 @@ int nh_solver_setup(Ctx* c) {
     const long long tw1 = g1 * NW1;
     int R1 = nny;
     long long best1 = -1;
-    for (int R = 4; R <= nny; ++R) {
+    for (int R = NH_MINROWS; R <= nny; ++R) {
       long long nb = (nny + R - 1) / R;
       long long rounds = (nstrips * nb + tw1 - 1) / tw1;
       long long cost = rounds * (R + 2);
       if (best1 < 0 || cost < best1) { best1 = cost; R1 = R; }
     }
-    if (nny < 4) R1 = nny;
+    if (nny < NH_MINROWS) R1 = nny;
     c->srj_grid = (int)g1; c->srj_R = R1; c->srj_nbands = (nny + R1 - 1) / R1;
     const int mmax = c->prm.srj_mmax;
     std::vector<double> tab((size_t)2 * mmax - 1);
@@ -1041,7 +883,7 @@ void nh_launch_solve(Ctx* c, const real* b, real* x, int count_stats) {
   P.count_stats = count_stats;
   void* args[] = {&P};
   NH_CUDA_OK(c, cudaLaunchCooperativeKernel((void*)k_bicgstab, dim3(c->solver_grid), dim3(NT), args,
-                                            NH_BULK ? (size_t)NW * RING_BYTES : 0, c->stream));
+                                            0, c->stream));
   c->launches++;
 }
 
