@@ -155,6 +155,38 @@ def whole_job_value(cells_per_replica, steps, world, seconds_max):
     return world * cells_per_replica * steps / seconds_max
 
 
+def _predictor_roofline(nh, prof, nc, args, hbm_peak, hbm_src):
+    """SWE mode: the dominant kernel is the fused predictor, bounded by the plain fp64 ALUs.
+    achieved = fp64-pipe warp instructions per second = (instructions per cell, ncu sm__inst_executed_pipe_fp64
+    of this kernel on this workload, profiles/traffic.json) x cells x launches / CUDA-event time of the launches;
+    peak = the fp64 FMA rate measured live by nh_fp64_rate (/ 32: warp instructions).  The HBM side (56 B per
+    cell) is reported beside it; the bound is the slower of the two."""
+    pm, pn = prof["predictor"]
+    rate = nh.fp64_rate() / 32.0
+    per_cell = None
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(tp):
+        try:
+            per_cell = json.load(open(tp)).get("predictor_fp64_pipe_warp_inst_per_cell", {}).get(
+                "f32" if args.precision == 32 else "f64")
+        except Exception:
+            pass
+    t = pm * 1e-3
+    hbm = 56.0 * (0.5 if args.precision == 32 else 1.0) * nc * pn / t / 1e9 if t > 0 else 0.0
+    out = {"bound": "alu", "kernel": "k_predictor (one launch per Runge-Kutta stage)", "unit": "fp64 warp-instructions/s",
+           "peak": rate, "peak_source": "measured live: nh_fp64_rate (DFMA chains), / 32",
+           "achieved": None, "frac": None, "traffic": None,
+           "fp64_pipe_warp_inst_per_cell": per_cell, "launches": pn, "avg_launch_ms": pm / max(pn, 1),
+           "cells_per_s_per_launch": nc * pn / t if t > 0 else None,
+           "hbm_side": {"bytes_per_cell": 56.0 * (0.5 if args.precision == 32 else 1.0), "achieved_GBs": hbm,
+                        "peak_GBs": hbm_peak, "frac": hbm / hbm_peak, "peak_source": hbm_src},
+           "phase_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()}}
+    if per_cell and t > 0:
+        out["achieved"] = per_cell * nc * pn / t
+        out["frac"] = out["achieved"] / rate
+    return out
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -210,6 +242,8 @@ def run_b200(args):
         prm.update(solver=1, srj_eps=args.srj_eps)
     if args.precision == 32:      # the optional fp32 variant: labelled, never the headline
         prm.update(precision=32, solver_rtol=1e-4)
+    if args.hydrostatic:          # SWE mode (nonhydro = 0): the step is the fused predictor alone (Table 2, column SWE)
+        prm.update(nonhydro=0)
     sim = nh.NH(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], stream=stream, **prm)
     sim.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
 
@@ -265,7 +299,10 @@ def run_b200(args):
                 traffic = traffic_unit * node_iters / max(sol_n, 1)
         except Exception:
             pass
-    roofline = {
+    if args.hydrostatic:
+        roofline = _predictor_roofline(nh, prof, nc, args, peak, peak_src)
+    else:
+      roofline = {
         "bound": "hbm", "kernel": ("k_srj" if args.solver == "srj" else "k_bicgstab") +
                                   " (one cooperative launch per pressure solve)",
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
@@ -281,7 +318,7 @@ def run_b200(args):
         "iterations_per_launch": (iters + solves) / max(solves, 1),
         "phase_ms_per_step": {k: v[0] / args.steps for k, v in prof.items()},
         "kernel_share_of_step": sol_ms / ms if ms > 0 else None,
-    }
+      }
 
     # ---- end-to-end leg: host buffers in and out through the C ABI every step
     hb = [{k: torch.empty(cfg[k].shape, dtype=torch.float64).pin_memory() for k in ("h", "qx", "qy", "w", "p")}
@@ -313,7 +350,8 @@ def run_b200(args):
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32" if args.precision == 32 else "f64", "data": "synthetic",
         "config": {"workload": f"configs[{args.config - 1}] {cfg['name']} {nx}x{ny} cells, dx={cfg['dx']} m"
-                               + (" -- fp32 VARIANT (precision = 32, solver_rtol 1e-4), not the fp64 headline" if args.precision == 32 else ""),
+                               + (" -- fp32 VARIANT (precision = 32, solver_rtol 1e-4), not the fp64 headline" if args.precision == 32 else "")
+                               + (" -- SWE MODE (nonhydro = 0: predictor only), not the headline" if args.hydrostatic else ""),
                    "solver": (("Jacobi-BiCGStab rtol %s, device-resident convergence" % ("1e-4" if args.precision == 32 else "1e-12")) if args.solver == "bicgstab"
                               else f"scheduled-relaxation Jacobi (paper's solver), increment rule (32) eps {args.srj_eps:g}"),
                    "iters_per_solve": iters / max(solves, 1), "time_order": 2,
@@ -611,6 +649,7 @@ def main():
     ap.add_argument("--parityruns", default="", help="idx:NXxNY:steps[:window],... : oracle beside the CUDA path over the "
                     "configured horizon, parity at 10 checkpoints (slow; a record for profiles/)")
     ap.add_argument("--rtol32", type=float, default=1e-4, help="--precision 32 with --parityruns: solver_rtol of the fp32 run")
+    ap.add_argument("--hydrostatic", action="store_true", help="SWE mode (nonhydro = 0): the predictor alone; alu-bound roofline")
     ap.add_argument("--onesolve", action="store_true", help="one isolated pressure solve after --warmup steps (ncu capture)")
     ap.add_argument("--param", action="append", default=[], help="--parityruns: override a parameter, key=value (repeatable)")
     ap.add_argument("--spread", action="store_true", help="--parityruns: also run a second oracle with a 10 x tighter "

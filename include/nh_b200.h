@@ -170,6 +170,12 @@ enum { NH_PROF_PREDICTOR = 0, NH_PROF_ASSEMBLY = 1, NH_PROF_SOLVER = 2, NH_PROF_
 int nh_profile(nh_ctx* ctx, int enable);
 int nh_profile_read(nh_ctx* ctx, double* ms, long long* groups);
 
+/* Measurement hook (bench.py's predictor roofline): the fp64 instruction rate of the current device,
+ * thread-level fused multiply-adds per second, measured with CUDA events on a kernel of independent
+ * DFMA chains (2 flops each; / 32 = warp instructions as ncu counts them).  Needs no context;
+ * synchronises.  dfma_per_second is a HOST pointer. */
+int nh_fp64_rate(void* cuda_stream, double* dfma_per_second);
+
 /* ---- test hooks (not on the timed path); node arrays in/out use the public node layout ---- */
 int nh_compute_dt(nh_ctx* ctx, double* dt_host);          /* CFL dt of the current state; synchronises */
 int nh_apply_A(nh_ctx* ctx, const double* x_nodes, double* y_nodes); /* y = A(h,z) x, matrix-free (S8) */

@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libnh_b200.so")
 KERNEL_SOURCES = ["nh_core.cu", "nh_predictor.cu", "nh_pressure.cu", "nh_solver.cu"]  # once per precision
-ABI_SOURCE = "nh_abi.cu"
+ABI_SOURCES = ["nh_abi.cu", "nh_peak.cu"]   # once
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-fmad=false", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-cudart", "shared"]
 OBJ = os.path.join(HERE, "build")
@@ -51,8 +51,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
         for src in KERNEL_SOURCES:
             obj = os.path.join(OBJ, f"{os.path.splitext(src)[0]}_{prec}.o")
             jobs.append((obj, common + [f"-DNH_PREC={prec}", "-o", obj, os.path.join(CSRC, src)]))
-    obj = os.path.join(OBJ, "nh_abi.o")
-    jobs.append((obj, common + ["-o", obj, os.path.join(CSRC, ABI_SOURCE)]))
+    for src in ABI_SOURCES:
+        obj = os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
+        jobs.append((obj, common + ["-o", obj, os.path.join(CSRC, src)]))
     procs = [(o, subprocess.Popen(cmd, cwd=HERE, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True))
              for o, cmd in jobs]
     failed = []

@@ -61,7 +61,7 @@ EXPORTS = (
     "nh_default_params", "nh_create", "nh_destroy", "nh_set_state", "nh_get_state", "nh_set_time", "nh_step",
     "nh_hydrostatic_step", "nh_nonhydro_correct", "nh_sync", "nh_get_info", "nh_last_error",
     "nh_launch_count", "nh_profile", "nh_profile_read", "nh_compute_dt", "nh_apply_A", "nh_coeffs",
-    "nh_rhs", "nh_constraint", "nh_solve", "nh_breaking", "nh_w_advect",
+    "nh_rhs", "nh_constraint", "nh_solve", "nh_breaking", "nh_w_advect", "nh_fp64_rate",
 )
 
 
@@ -102,8 +102,18 @@ def lib():
         L.nh_solve.argtypes = [_vp, _vp, _vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
         L.nh_breaking.argtypes = [_vp, C.c_double, _vp, _vp, _vp]
         L.nh_w_advect.argtypes = [_vp, C.c_double, _vp]
+        L.nh_fp64_rate.argtypes = [_vp, C.POINTER(C.c_double)]
         _lib = L
     return _lib
+
+
+def fp64_rate(stream=None) -> float:
+    """Measured fp64 FMA rate of the current device (thread instructions per second)."""
+    r = C.c_double()
+    st = lib().nh_fp64_rate(None if stream is None else stream.cuda_stream, C.byref(r))
+    if st != OK:
+        raise NHError(st, "nh_fp64_rate")
+    return r.value
 
 
 def default_params(**kw) -> Params:
