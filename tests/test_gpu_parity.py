@@ -250,8 +250,12 @@ def test_config3_radial_reduced(O, G):
 
 
 def test_config4_beach_reduced(O, G):
-    # shorter and narrower beach: same dx, slope, generating zone, breaking parameters
-    cfg, o, g = run_config(O, G, 4, 300, checkpoints=3, nx=640, ny=8)
+    # shorter and narrower beach: same dx, slope, generating zone, breaking parameters.  180 steps: two
+    # ORACLE runs at solver_rtol 1e-12 and 1e-13 agree to 0.04 bars at step 200 of this strip and have
+    # drifted to 0.6 - 1.9 bars by step 400 (profiles/r02b: the run is sensitive to solver-level
+    # differences), so a longer window at the 1e-9 bars would test luck, not parity; the full
+    # horizon is compared bit for bit under solver 1 (tests/test_gpu_horizon.py)
+    cfg, o, g = run_config(O, G, 4, 180, checkpoints=3, nx=640, ny=8)
     # Clamps here are round-off events (|h*| ~ 1e-17 < 0 in dry shoreline cells, driven by the
     # 1e-12-level solver noise that the elliptic solve spreads to the still shoreline), so their
     # count is not unique across two valid solves (R7/R23): compare the state (above),
@@ -736,3 +740,21 @@ def test_conical_island_reduced(O, G, adv):
     g.step(15)
     assert g.sync() == 0
     assert_parity(g.get_state(), o.get_state(), cfg["H"], cfg["h0"])
+
+
+def test_set_state_after_a_step_starts_the_cfl_reduction_from_zero(O, G):
+    # the RK combine leaves the CFL rate of ITS state on the device; a state set afterwards must get the
+    # time step of eq. (23) of the new state alone (the max-reduction restarts from zero)
+    fast = rnd_cfg(70, 37, BCS[1], seed=5, dry=0.0)
+    slow = rnd_cfg(70, 37, BCS[1], seed=5, dry=0.0)
+    slow["qx"] = 0.01 * slow["qx"]; slow["qy"] = 0.01 * slow["qy"]; slow["h"] = 0.25 * slow["h"] + 0.0
+    slow["h"] = np.maximum(slow["h"], 0.0)
+    o, g = both(O, G, fast)
+    g.step(2)
+    assert g.sync() == 0
+    g.set_state(slow["h"], slow["qx"], slow["qy"], slow["w"], slow["p"])
+    o.set_state(slow["h"], slow["qx"], slow["qy"], slow["w"], slow["p"])
+    assert g.compute_dt() == o.compute_dt()
+    g.step(1)
+    o.step(1)
+    assert g.sync() == 0 and g.info().dt_last == o.info().dt_last
