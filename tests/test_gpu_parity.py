@@ -250,12 +250,19 @@ def test_config3_radial_reduced(O, G):
 
 
 def test_config4_beach_reduced(O, G):
-    # shorter and narrower beach: same dx, slope, generating zone, breaking parameters.  180 steps: two
-    # ORACLE runs at solver_rtol 1e-12 and 1e-13 agree to 0.04 bars at step 200 of this strip and have
-    # drifted to 0.6 - 1.9 bars by step 400 (profiles/r02b: the run is sensitive to solver-level
-    # differences), so a longer window at the 1e-9 bars would test luck, not parity; the full
-    # horizon is compared bit for bit under solver 1 (tests/test_gpu_horizon.py)
-    cfg, o, g = run_config(O, G, 4, 180, checkpoints=3, nx=640, ny=8)
+    # shorter and narrower beach: same dx, slope, generating zone, breaking parameters.  The run is
+    # sensitive to solver-level differences in two phases (profiles/r02b, `--parityruns 4:640x8:300
+    # --spread`): while the foot of the generated wave (eta ~ 1e-3 m) crosses the still shoreline
+    # cells (steps 30-90: two ORACLE runs at solver_rtol 1e-12 and 1e-13 differ by up to 1e3 bars in
+    # q), and again from step ~270 on.  In between both pairs agree to <= 0.1 bars: compared there.
+    # The full horizon is compared bit for bit under solver 1 (tests/test_gpu_horizon.py).
+    cfg = inputs.make_config(4, nx=640, ny=8)
+    o, g = both(O, G, cfg)
+    for n in (120, 30, 30, 30):
+        o.step(n)
+        g.step(n)
+        assert g.sync() == 0
+        assert_parity(g.get_state(), o.get_state(), cfg["H"], cfg["h0"])
     # Clamps here are round-off events (|h*| ~ 1e-17 < 0 in dry shoreline cells, driven by the
     # 1e-12-level solver noise that the elliptic solve spreads to the still shoreline), so their
     # count is not unique across two valid solves (R7/R23): compare the state (above),
