@@ -469,8 +469,8 @@ def test_manning_beach_reduced_parity(O, G):
             assert np.array_equal(so[k], sg[k]), (k, np.max(np.abs(so[k] - sg[k])))
     assert o.info().iters_total == g.info().iters_total > 0
     o, g = both(O, G, cfg, manning_n=0.01)
-    o.step(20)
-    g.step(20)
+    o.step(15)
+    g.step(15)
     assert g.sync() == 0
     assert_parity(g.get_state(), o.get_state(), cfg["H"], cfg["h0"])
 
