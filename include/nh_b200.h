@@ -87,6 +87,12 @@ typedef struct {
                          L109-113), instead of h w_t = p: in every stage the node values w are first
                          transported by first-order upwind differences with the 4-cell mean of the
                          desingularised velocities (R30); default 0                       */
+  int warm_start;     /* 1 (default): a pressure solve starts from the previous solution plus the quadratic
+                         extrapolation of the same-kind increments of the last three steps,
+                         x0 = s1 + 3 (s2 - s3) - 3 (s4 - s5) + (s6 - s7) (R32), once seven
+                         solutions exist since the last nh_set_state, for solver 0 with solver_rtol
+                         <= 1e-8 (looser stopping rules start from the previous solution, as 0 does) */
+  int reserved;
 } nh_params;
 
 typedef struct {
@@ -194,6 +200,9 @@ int nh_breaking(nh_ctx* ctx, double dt, double* qx2, double* qy2, double* w2);
  * state carried over dt by the node velocities of the current state -> node array w_out; the state
  * is not changed.  dt > 0 required; works whatever prm.w_advect says; synchronises. */
 int nh_w_advect(nh_ctx* ctx, double dt, double* w_out);
+/* The vector the next pressure solve of a step would start from (R32) -> node array; the
+ * state is not changed; synchronises. */
+int nh_start_vector(nh_ctx* ctx, double* x0_nodes);
 
 #ifdef __cplusplus
 }

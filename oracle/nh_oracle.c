@@ -47,6 +47,8 @@ struct nho_ctx {
   /* RK copies */
   double *h0, *qx0, *qy0, *w0;
   double *wadv;              /* w after the transport step of the w-advection variant (R30) */
+  double *hist[7];           /* R32: the last seven pressure solutions, hist[0] the most recent */
+  int nhist;                 /* how many of them are valid (reset by nho_set_state) */
 };
 
 /* ------------------------------------------------------------------------------------ */
@@ -920,6 +922,37 @@ static void w_advection(nho_ctx* c, const double* w_in, double dt, double* w_out
     }
 }
 
+/* Reading R32: the start vector of a pressure solve.  The paper does not say where its iteration
+ * starts; R14 took the previous solution.  The solves of a run alternate between the two Runge-Kutta
+ * stages, and the increment from one solve to the next, i_k = s_k - s_(k-1), repeats every second
+ * solve up to a slow drift in time.  With warm_start = 1 (default) the start vector is the previous
+ * solution plus the quadratic extrapolation of the same-kind increments of the last three steps,
+ *     x0 = s1 + 3 (s2 - s3) - 3 (s4 - s5) + (s6 - s7)      (s1 = most recent solution),
+ * once seven solutions exist since the last nho_set_state and only for solver 0 with solver_rtol <= 1e-8;
+ * otherwise, and with warm_start = 0, x0 = p as it stands (the previous solution, or what nho_set_state gave).  A start vector does not
+ * change what the solve converges to (stopping rule unchanged); it saves 16-27 % of the iterations
+ * on the five configs (R32). */
+static void start_vector(const nho_ctx* c, double* x0) {
+  /* only where the stored solutions are accurate enough to be extrapolated: the formula amplifies
+   * their error 15-fold, so with a loose stopping rule (solver 1 at the paper's eps, tolerances above
+   * 1e-8) the plain previous solution is the better start (measured: DESIGN.md R32) */
+  if (!c->prm.warm_start || c->prm.solver != 0 || c->prm.solver_rtol > 1e-8 || c->nhist < 7) return;
+  double* const* h = c->hist;
+  for (int J = 0; J < c->nny; ++J)
+    for (int I = 0; I < c->nnx; ++I) {
+      size_t k = NIDX(c, I, J);
+      x0[k] = ((h[0][k] + 3.0 * (h[1][k] - h[2][k])) - 3.0 * (h[3][k] - h[4][k])) + (h[5][k] - h[6][k]);
+    }
+}
+static void push_solution(nho_ctx* c, const double* x) {
+  size_t nn = (size_t)(c->nx + 1) * (size_t)(c->ny + 1);
+  double* t = c->hist[6];
+  for (int a = 6; a > 0; --a) c->hist[a] = c->hist[a - 1];
+  c->hist[0] = t;
+  memcpy(c->hist[0], x, nn * sizeof(double));
+  if (c->nhist < 7) c->nhist++;
+}
+
 /* S6-S10 on U* = (h1,qx1,qy1) with w_in; results to (qx_out,qy_out,w_out), p in c->p. */
 static int nonhydro_part(nho_ctx* c, const double* w_in, double dt, double* qx_out, double* qy_out,
                          double* w_out) {
@@ -939,7 +972,9 @@ static int nonhydro_part(nho_ctx* c, const double* w_in, double dt, double* qx_o
       c->b[NIDX(c, I, J)] = (dt > 0.0) ? -node_B(c, c->h1, c->qx2, c->qy2, c->z, c->w2, I, J) / dt
                                        : 0.0;   /* R26: all-dry domain, dt = 0 => p~ = 0 */
   int iters = 0; double relres = 0.0;
+  start_vector(c, c->p);   /* R32 */
   int st = solve_system(c, c->h1, c->z, c->b, c->p, &iters, &relres);
+  push_solution(c, c->p);
   c->info.iters_last = iters;
   c->info.iters_total += iters;
   c->info.solves += 1;
@@ -982,7 +1017,7 @@ void nho_default_params(nho_params* prm) {
   prm->breaking = 0; prm->nonhydro = 1; prm->time_order = 2; prm->space_order = 2;
   prm->bc_xlo = prm->bc_xhi = prm->bc_ylo = prm->bc_yhi = NHO_BC_OUTFLOW;
   prm->solver_maxit = 10000; prm->gen_on = 0; prm->precision = 64;
-  prm->solver = 0; prm->srj_eps = 1e-5; prm->srj_mmax = 256;
+  prm->solver = 0; prm->srj_eps = 1e-5; prm->srj_mmax = 256; prm->warm_start = 1;
 }
 
 static int bc_ok(int b) { return b == NHO_BC_PERIODIC || b == NHO_BC_WALL || b == NHO_BC_OUTFLOW; }
@@ -1003,6 +1038,7 @@ int nho_create(nho_ctx** out, int nx, int ny, double dx, double dy, const double
   if (!(prm->manning_n >= 0.0)) return NHO_EINVAL;
   if (prm->solver != 0 && prm->solver != 1) return NHO_EINVAL;
   if (prm->w_advect != 0 && prm->w_advect != 1) return NHO_EINVAL;
+  if (prm->warm_start != 0 && prm->warm_start != 1) return NHO_EINVAL;
   if (!(prm->srj_rel >= 0.0)) return NHO_EINVAL;
   if (!(prm->abs_xlo >= 0.0) || !(prm->abs_xhi >= 0.0) || !(prm->abs_ylo >= 0.0) || !(prm->abs_yhi >= 0.0)) return NHO_EINVAL;
   if ((prm->abs_xlo > 0.0 || prm->abs_xhi > 0.0) && prm->bc_xlo == NHO_BC_PERIODIC) return NHO_EINVAL;
@@ -1022,7 +1058,8 @@ int nho_create(nho_ctx** out, int nx, int ny, double dx, double dy, const double
   double** cellp[] = { &c->H, &c->h, &c->qx, &c->qy, &c->eta, &c->u, &c->v, &c->h1, &c->qx1, &c->qy1,
                        &c->qx2, &c->qy2, &c->z, &c->h0, &c->qx0, &c->qy0 };
   double** nodep[] = { &c->w, &c->p, &c->w2, &c->b, &c->kr, &c->kr0, &c->kp, &c->kv, &c->ks, &c->kt,
-                       &c->kph, &c->ksh, &c->kdiag, &c->w0, &c->wadv };
+                       &c->kph, &c->ksh, &c->kdiag, &c->w0, &c->wadv, &c->hist[0], &c->hist[1], &c->hist[2],
+                       &c->hist[3], &c->hist[4], &c->hist[5], &c->hist[6] };
   int ok = 1;
   for (size_t a = 0; a < sizeof(cellp) / sizeof(cellp[0]); ++a) { *cellp[a] = (double*)calloc(nc, sizeof(double)); if (!*cellp[a]) ok = 0; }
   for (size_t a = 0; a < sizeof(nodep) / sizeof(nodep[0]); ++a) { *nodep[a] = (double*)calloc(nn, sizeof(double)); if (!*nodep[a]) ok = 0; }
@@ -1038,7 +1075,8 @@ void nho_destroy(nho_ctx* c) {
   if (!c) return;
   double* all[] = { c->H, c->h, c->qx, c->qy, c->eta, c->u, c->v, c->h1, c->qx1, c->qy1, c->qx2, c->qy2,
                     c->z, c->h0, c->qx0, c->qy0, c->w, c->p, c->w2, c->b, c->kr, c->kr0, c->kp, c->kv,
-                    c->ks, c->kt, c->kph, c->ksh, c->kdiag, c->w0, c->wadv };
+                    c->ks, c->kt, c->kph, c->ksh, c->kdiag, c->w0, c->wadv, c->hist[0], c->hist[1], c->hist[2],
+                    c->hist[3], c->hist[4], c->hist[5], c->hist[6] };
   for (size_t a = 0; a < sizeof(all) / sizeof(all[0]); ++a) free(all[a]);
   free(c->flag_c); free(c->flag_n);
   free(c);
@@ -1074,6 +1112,7 @@ int nho_set_state(nho_ctx* c, const double* h, const double* qx, const double* q
   memcpy(c->qy, qy, nc * sizeof(double));
   nodes_in(c, w, c->w);
   nodes_in(c, p, c->p);
+  c->nhist = 0;   /* R32: the solution history belongs to the replaced state */
   return NHO_OK;
 }
 
@@ -1229,6 +1268,15 @@ int nho_w_advect(nho_ctx* c, double dt, double* w_out) {
   derived_fields(c, c->h, c->qx, c->qy);
   w_advection(c, c->w, dt, c->wadv);
   nodes_out(c, c->wadv, w_out);
+  return NHO_OK;
+}
+
+int nho_start_vector(nho_ctx* c, double* x0_nodes) {
+  if (!c || !x0_nodes) return NHO_EINVAL;
+  size_t nn = (size_t)(c->nx + 1) * (size_t)(c->ny + 1);
+  memcpy(c->kr, c->p, nn * sizeof(double));
+  start_vector(c, c->kr);
+  nodes_out(c, c->kr, x0_nodes);
   return NHO_OK;
 }
 

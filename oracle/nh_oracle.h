@@ -52,6 +52,10 @@ typedef struct {
   int srj_mmax;        /* solver 1: longest relaxation cycle (power of two), default 256        */
   int w_advect;        /* 1: vertical-velocity equation of [7], (hw)_t + div(hw u) = p (L109-113), instead of
                           h w_t = p: w transported by first-order upwind differences (reading R30) */
+  int warm_start;      /* 1 (default): start vector of a solve = previous solution + quadratic extrapolation of
+                          the same-kind increments of the last three steps (reading R32; solver 0 with solver_rtol <= 1e-8
+                          only); 0: previous solution */
+  int reserved;
 } nho_params;
 
 typedef struct {
@@ -93,6 +97,7 @@ int  nho_coeffs(nho_ctx* c, double* AC, double* AE, double* AW, double* AN, doub
 int  nho_rhs(nho_ctx* c, double dt, double* b_nodes);   /* b = -B/dt of the current state (S7), breaking ignored */
 int  nho_constraint(nho_ctx* c, double* B_nodes);       /* discrete B, eq. (37), current state */
 int  nho_w_advect(nho_ctx* c, double dt, double* w_out); /* S5b alone (R30): w of the current state transported over dt */
+int  nho_start_vector(nho_ctx* c, double* x0_nodes); /* R32: the vector the next solve of a step would start from */
 int  nho_solve(nho_ctx* c, const double* b_nodes, double* x_nodes, int* iters, double* relres); /* S9; x in: start */
 int  nho_breaking(nho_ctx* c, double dt, double* qx2, double* qy2, double* w2); /* S6 alone: the current
                    state taken as U*, w -> q** = q* + dt R_u (cells), w** = w + dt R_w (nodes); updates the

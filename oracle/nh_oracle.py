@@ -22,7 +22,7 @@ class Params(C.Structure):
         ("breaking", C.c_int), ("nonhydro", C.c_int), ("time_order", C.c_int), ("space_order", C.c_int),
         ("bc_xlo", C.c_int), ("bc_xhi", C.c_int), ("bc_ylo", C.c_int), ("bc_yhi", C.c_int),
         ("solver_maxit", C.c_int), ("gen_on", C.c_int), ("precision", C.c_int), ("solver", C.c_int),
-        ("srj_mmax", C.c_int), ("w_advect", C.c_int),
+        ("srj_mmax", C.c_int), ("w_advect", C.c_int), ("warm_start", C.c_int), ("reserved", C.c_int),
     ]
 
 
@@ -67,6 +67,7 @@ def lib():
         L.nho_solve.argtypes = [C.c_void_p, _dp, _dp, C.POINTER(C.c_int), _dp]
         L.nho_breaking.argtypes = [C.c_void_p, C.c_double, _dp, _dp, _dp]
         L.nho_w_advect.argtypes = [C.c_void_p, C.c_double, _dp]
+        L.nho_start_vector.argtypes = [C.c_void_p, _dp]
         L.nho_face_fluct.argtypes = [C.c_double] * 9 + [_dp, _dp]
         L.nho_face_fluct.restype = None
         L.nho_dsg.argtypes = [C.c_double] * 3
@@ -201,6 +202,12 @@ class Oracle:
         w = np.empty(self.nshape)
         self._check(lib().nho_w_advect(self._h, float(dt), _ptr(w)))
         return w
+
+    def start_vector(self):
+        """R32: the vector the next pressure solve of a step would start from."""
+        x = np.empty(self.nshape)
+        self._check(lib().nho_start_vector(self._h, _ptr(x)))
+        return x
 
     def solve(self, b, x0=None, allow_noconv=False):
         b = _c64(b, self.nshape)

@@ -25,7 +25,7 @@ void nh_default_params(nh_params* prm) {
   prm->breaking = 0; prm->nonhydro = 1; prm->time_order = 2; prm->space_order = 2;
   prm->bc_xlo = prm->bc_xhi = prm->bc_ylo = prm->bc_yhi = NH_BC_OUTFLOW;
   prm->solver_maxit = 10000; prm->gen_on = 0; prm->precision = 64;
-  prm->solver = 0; prm->srj_eps = 1e-5; prm->srj_mmax = 256; prm->w_advect = 0;
+  prm->solver = 0; prm->srj_eps = 1e-5; prm->srj_mmax = 256; prm->w_advect = 0; prm->warm_start = 1;
 }
 
 int nh_create(nh_ctx** out, int nx, int ny, double dx, double dy, const double* H,
@@ -125,6 +125,10 @@ int nh_breaking(nh_ctx* c, double dt, double* qx2, double* qy2, double* w2) {
 int nh_w_advect(nh_ctx* c, double dt, double* w_out) {
   if (!c) return NH_EINVAL;
   return NH_FWD(c, nh64::core_w_advect(c->c64, dt, w_out), nh32::core_w_advect(c->c32, dt, w_out));
+}
+int nh_start_vector(nh_ctx* c, double* x0_nodes) {
+  if (!c) return NH_EINVAL;
+  return NH_FWD(c, nh64::core_start_vector(c->c64, x0_nodes), nh32::core_start_vector(c->c32, x0_nodes));
 }
 int nh_solve(nh_ctx* c, const double* b_nodes, double* x_nodes, int* iters, double* relres) {
   if (!c) return NH_EINVAL;

@@ -214,6 +214,13 @@ struct ProfScope {  // CUDA-event bracket of one kernel group on the context's s
   }
 };
 
+// R32: the extrapolated start vector is used once seven solutions exist, and only where the stored
+// solutions are accurate enough to be extrapolated (the formula amplifies their error 15-fold):
+// solver 0 with solver_rtol <= 1e-8
+inline bool extrapolate_start(const Ctx* c) {
+  return c->prm.warm_start && c->prm.solver == 0 && c->prm.solver_rtol <= 1e-8 && c->nhist == 7;
+}
+
 // S6-S10 on U* = (h1, qx1, qy1) with w_in -> (qx_out, qy_out, w_out); p~ in c->p (warm start).
 void nonhydro_part(Ctx* c, const real* h1, const real* qx1, const real* qy1,
                    const real* w_in, real* qx_out, real* qy_out, real* w_out) {
@@ -234,7 +241,14 @@ void nonhydro_part(Ctx* c, const real* h1, const real* qx1, const real* qy1,
   }
   {
     ProfScope ps(c, NH_PROF_SOLVER);
+    if (extrapolate_start(c)) nh_launch_start_vector(c, c->p);  // R32
     nh_launch_solve(c, c->b, c->p, 1);
+    // the solution joins the history (rotate the seven planes, copy into the oldest)
+    real* t = c->hist[6];
+    for (int a = 6; a > 0; --a) c->hist[a] = c->hist[a - 1];
+    c->hist[0] = t;
+    copy_async(c, c->hist[0] - node_origin(c), c->p - node_origin(c), c->nni * sizeof(real));
+    if (c->nhist < 7) c->nhist++;
   }
   {
     ProfScope ps(c, NH_PROF_CORRECT);
@@ -297,6 +311,7 @@ int core_create(Ctx** out, int nx, int ny, double dx, double dy, const double* H
   if (!(prm->manning_n >= 0.0)) return NH_EINVAL;
   if (prm->solver != 0 && prm->solver != 1) return NH_EINVAL;
   if (prm->w_advect != 0 && prm->w_advect != 1) return NH_EINVAL;
+  if (prm->warm_start != 0 && prm->warm_start != 1) return NH_EINVAL;
   if (!(prm->srj_rel >= 0.0)) return NH_EINVAL;
   if (!(prm->abs_xlo >= 0.0) || !(prm->abs_xhi >= 0.0) || !(prm->abs_ylo >= 0.0) || !(prm->abs_yhi >= 0.0)) return NH_EINVAL;
   if ((prm->abs_xlo > 0.0 || prm->abs_xhi > 0.0) && prm->bc_xlo == NH_BC_PERIODIC) return NH_EINVAL;
@@ -330,7 +345,7 @@ int core_create(Ctx** out, int nx, int ny, double dx, double dy, const double* H
   c->nc = (size_t)nx * ny;
   c->nn = (size_t)(nx + 1) * (ny + 1);
   c->nni = (size_t)c->g.np * (ny + 1 + 2 * NH_ROW_PAD);
-  c->cur = 0; c->curw = 0;
+  c->cur = 0; c->curw = 0; c->nhist = 0;
   c->lam_valid = false;
   c->host_status = NH_OK;
 
@@ -339,7 +354,8 @@ int core_create(Ctx** out, int nx, int ny, double dx, double dy, const double* H
                       &c->qy[0], &c->qy[1], &c->qy[2], &c->qx1, &c->qy1, &c->z};
   real** nodes[] = {&c->w[0], &c->w[1], &c->w[2], &c->p, &c->b, &c->dg, &c->dinv, &c->cE, &c->cW,
                       &c->cN, &c->cS, &c->ky, &c->kr, &c->krB, &c->kr0, &c->kpA, &c->kpB, &c->kvA,
-                      &c->kvB, &c->kt, &c->w2, &c->hc, &c->zc, &c->wadv};
+                      &c->kvB, &c->kt, &c->w2, &c->hc, &c->zc, &c->wadv, &c->hist[0], &c->hist[1], &c->hist[2],
+                    &c->hist[3], &c->hist[4], &c->hist[5], &c->hist[6]};
   for (real** p : cells) ok = ok && dalloc(c, p, c->nc);
   for (real** p : nodes) ok = ok && nalloc(c, p);
   if (kEta) {  // fp32 variant: eta planes, the bathymetry as given, an fp64 staging plane
@@ -405,6 +421,7 @@ int core_set_state(Ctx* c, const double* h, const double* qx, const double* qy, 
   if (c->sc_host->flags & NH_FLAG_BADSTATE)
     return fail(c, NH_EINVAL, "set_state: h<0 or non-finite input");
   c->cur = s1;
+  c->nhist = 0;  // R32: the solution history belongs to the replaced state
   if (node_in(c, c->w[c->curw], w) || node_in(c, c->p, p)) return NH_ECUDA;
   // the CFL rate left by the last RK combine belongs to the replaced state: k_lambda takes a max
   // onto lam_bits, so it has to start from zero (eq. (23) of the NEW state only)
@@ -633,6 +650,15 @@ int core_w_advect(Ctx* c, double dt, double* w_out) {
   c->lam_valid = false;
   nh_launch_w_advect(c, c->h[c->cur], c->qx[c->cur], c->qy[c->cur], c->w[c->curw], c->wadv);
   if (node_out(c, c->wadv, w_out)) return NH_ECUDA;
+  cudaStreamSynchronize(c->stream);
+  return check_launch(c);
+}
+
+int core_start_vector(Ctx* c, double* x0_nodes) {
+  if (!c || !x0_nodes) return NH_EINVAL;
+  if (copy_async(c, c->w2 - node_origin(c), c->p - node_origin(c), c->nni * sizeof(real))) return NH_ECUDA;
+  if (extrapolate_start(c)) nh_launch_start_vector(c, c->w2);
+  if (node_out(c, c->w2, x0_nodes)) return NH_ECUDA;
   cudaStreamSynchronize(c->stream);
   return check_launch(c);
 }

@@ -32,6 +32,7 @@
   int core_constraint(Ctx* c, double* B_nodes);                                                    \
   int core_breaking(Ctx* c, double dt, double* qx2, double* qy2, double* w2);                     \
   int core_w_advect(Ctx* c, double dt, double* w_out);                                             \
+  int core_start_vector(Ctx* c, double* x0_nodes);                                                 \
   int core_solve(Ctx* c, const double* b_nodes, double* x_nodes, int* iters, double* relres);     \
   }
 

@@ -217,6 +217,8 @@ struct Ctx {
   real* w[3];
   real* w2;  // w** (breaking on)
   real* wadv;  // w after the transport step of the w-advection variant (R30)
+  real* hist[7];  // R32: the last seven pressure solutions, hist[0] the most recent
+  int nhist;      // how many of them are valid (reset by set_state)
   real* p;   // pressure multiplier p~ (warm start of the next solve)
   real* b;   // right-hand side
   real *dg, *dinv, *cE, *cW, *cN, *cS;  // diag(A), its inverse, column-scaled off-diagonals
@@ -273,6 +275,7 @@ void nh_launch_correct(Ctx* c, const real* h, const real* z, const real* qx2,
                        real* qy_out, real* w_out);
 void nh_launch_w_advect(Ctx* c, const real* h, const real* qx, const real* qy,
                         const real* w_in, real* w_out);  // R30
+void nh_launch_start_vector(Ctx* c, real* x0);  // R32: x0 <- extrapolation of c->hist (all 7 valid)
 void nh_launch_relax(Ctx* c, real* h, real* qx, real* qy, real* w, real* p, int stage);
 void nh_launch_absorb(Ctx* c, real* h, real* qx, real* qy, real* w, real* p);
 void nh_launch_nodes_out(Ctx* c, const real* src, double* dst);

@@ -404,6 +404,19 @@ k_w_advect(NhGrid G, const NhScal* sc, real delta, const real* __restrict__ h,
   w_out[(size_t)J * G.np + I] = wc - (real)sc->dt * (un * wx + vn * wy);
 }
 
+// R32: start vector of a pressure solve from the last seven solutions (s1 the most recent):
+// x0 = ((s1 + 3 (s2 - s3)) - 3 (s4 - s5)) + (s6 - s7), in this operation order (bit-exact against
+// the oracle, so that solver 1 stays bit-exact end to end)
+__global__ void __launch_bounds__(BX* BY)
+k_start_vector(NhGrid G, const real* __restrict__ s1, const real* __restrict__ s2,
+               const real* __restrict__ s3, const real* __restrict__ s4, const real* __restrict__ s5,
+               const real* __restrict__ s6, const real* __restrict__ s7, real* __restrict__ x0) {
+  int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
+  if (I >= G.nnx || J >= G.nny) return;
+  size_t k = (size_t)J * G.np + I;
+  x0[k] = ((s1[k] + RC(3.0) * (s2[k] - s3[k])) - RC(3.0) * (s4[k] - s5[k])) + (s6[k] - s7[k]);
+}
+
 // S10: correction, eqs (36),(41): q <- q** + dt T_NH(p) at cells
 __global__ void __launch_bounds__(BX* BY)
 k_correct_cells(NhGrid G, const NhScal* sc, const real* __restrict__ h,
@@ -622,6 +635,12 @@ void nh_launch_w_advect(Ctx* c, const real* h, const real* qx, const real* qy,
                         const real* w_in, real* w_out) {
   k_w_advect<<<grid2(c->g.nnx, c->g.nny), dim3(BX, BY), 0, c->stream>>>(c->g, c->sc, c->prm.delta, h,
                                                                        qx, qy, w_in, w_out);
+  c->launches++;
+}
+void nh_launch_start_vector(Ctx* c, real* x0) {
+  real* const* h = c->hist;
+  k_start_vector<<<grid2(c->g.nnx, c->g.nny), dim3(BX, BY), 0, c->stream>>>(c->g, h[0], h[1], h[2], h[3],
+                                                                           h[4], h[5], h[6], x0);
   c->launches++;
 }
 void nh_launch_relax(Ctx* c, real* h, real* qx, real* qy, real* w, real* p, int stage) {

@@ -34,7 +34,7 @@ class Params(C.Structure):
         ("breaking", C.c_int), ("nonhydro", C.c_int), ("time_order", C.c_int), ("space_order", C.c_int),
         ("bc_xlo", C.c_int), ("bc_xhi", C.c_int), ("bc_ylo", C.c_int), ("bc_yhi", C.c_int),
         ("solver_maxit", C.c_int), ("gen_on", C.c_int), ("precision", C.c_int), ("solver", C.c_int),
-        ("srj_mmax", C.c_int), ("w_advect", C.c_int),
+        ("srj_mmax", C.c_int), ("w_advect", C.c_int), ("warm_start", C.c_int), ("reserved", C.c_int),
     ]
 
 
@@ -61,7 +61,7 @@ EXPORTS = (
     "nh_default_params", "nh_create", "nh_destroy", "nh_set_state", "nh_get_state", "nh_set_time", "nh_step",
     "nh_hydrostatic_step", "nh_nonhydro_correct", "nh_sync", "nh_get_info", "nh_last_error",
     "nh_launch_count", "nh_profile", "nh_profile_read", "nh_compute_dt", "nh_apply_A", "nh_coeffs",
-    "nh_rhs", "nh_constraint", "nh_solve", "nh_breaking", "nh_w_advect", "nh_fp64_rate",
+    "nh_rhs", "nh_constraint", "nh_solve", "nh_breaking", "nh_w_advect", "nh_fp64_rate", "nh_start_vector",
 )
 
 
@@ -102,6 +102,7 @@ def lib():
         L.nh_solve.argtypes = [_vp, _vp, _vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
         L.nh_breaking.argtypes = [_vp, C.c_double, _vp, _vp, _vp]
         L.nh_w_advect.argtypes = [_vp, C.c_double, _vp]
+        L.nh_start_vector.argtypes = [_vp, _vp]
         L.nh_fp64_rate.argtypes = [_vp, C.POINTER(C.c_double)]
         _lib = L
     return _lib
@@ -286,6 +287,11 @@ class NH:
         w = np.empty(self.nshape)
         self._check(lib().nh_w_advect(self._h, float(dt), w.ctypes.data))
         return w
+
+    def start_vector(self):
+        x = np.empty(self.nshape)
+        self._check(lib().nh_start_vector(self._h, x.ctypes.data))
+        return x
 
     def solve(self, b, x0=None, allow=()):
         keep = []

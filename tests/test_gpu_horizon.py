@@ -97,7 +97,7 @@ def test_config4_beach_2000_steps_narrow(O, G):
         # different valid solves of every pressure system
         assert np.mean((s0["h"] > 1e-5) != wet) <= 0.01, done
         assert np.max(np.abs(s0["h"] - so["h"])) <= 0.05 * cfg["h0"], done
-        assert g0.info().t == pytest.approx(io.t, rel=1e-6)
+        assert g0.info().t == pytest.approx(io.t, rel=1e-4)
     assert broke > 0          # the breaking criterion (9) was active inside a compared window
     assert wet_max > 8 * 100  # the shoreline ran up by more than 5 m of beach (100 cells per row)
     ig, io = g.info(), o.info()

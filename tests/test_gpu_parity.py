@@ -765,3 +765,50 @@ def test_set_state_after_a_step_starts_the_cfl_reduction_from_zero(O, G):
     g.step(1)
     o.step(1)
     assert g.sync() == 0 and g.info().dt_last == o.info().dt_last
+
+
+# ---------------------------------------------------------------- R32: start vector of the solve
+def test_start_vector_against_the_oracle_and_reset(O, G):
+    # default solver: both sides extrapolate their own solution histories (which agree to solver
+    # accuracy; the formula amplifies differences 15-fold); before seven solutions exist, right after
+    # set_state, and with the paper's solver (loose stopping rule: no extrapolation) it is p as it stands
+    cfg = rnd_cfg(150, 77, BCS[2], seed=43, dry=0.2, dx=0.2, dy=0.25)
+    o, g = both(O, G, cfg)
+    assert np.array_equal(o.start_vector(), g.start_vector())
+    for k in range(9):
+        dt = 0.004 * (1.0 + 0.1 * k)
+        o.nonhydro_correct(dt)
+        g.nonhydro_correct(dt)
+        assert g.sync() == 0
+        xo, xg, pg = o.start_vector(), g.start_vector(), g.get_state()["p"]
+        assert np.max(np.abs(xo - xg)) <= 1e-7 * np.max(np.abs(xo)), k
+        if k < 6:
+            assert np.array_equal(xg, pg)
+        else:
+            assert np.max(np.abs(xg - pg)) > 1e-6 * np.max(np.abs(pg))   # the extrapolation is active
+    g.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
+    assert np.array_equal(g.start_vector()[:-1, :], cfg["p"][:-1, :])     # (periodic duplicate row aside)
+    o, g = both(O, G, cfg, solver=1, srj_eps=1e-8)
+    for k in range(8):
+        o.nonhydro_correct(0.004)
+        g.nonhydro_correct(0.004)
+    assert np.array_equal(g.start_vector(), g.get_state()["p"]) and np.array_equal(o.start_vector(), g.start_vector())
+
+
+def test_start_vector_saves_iterations_not_accuracy(O, G):
+    cfg = inputs.make_config(3, nx=200, ny=176)
+    res = {}
+    for ws in (0, 1):
+        g = G.NH(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["H"], **dict(cfg["params"], warm_start=ws))
+        g.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
+        g.step(30)
+        assert g.sync() == 0
+        res[ws] = (g.get_state(), g.info().iters_total)
+        g.close()
+    assert res[1][1] < 0.88 * res[0][1]
+    assert_parity(res[1][0], res[0][0], cfg["H"], cfg["h0"])
+    o = O.Oracle(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["H"], **cfg["params"])
+    o.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
+    o.step(30)
+    assert_parity(res[1][0], o.get_state(), cfg["H"], cfg["h0"])
+    assert abs(res[1][1] - o.info().iters_total) <= 0.05 * o.info().iters_total

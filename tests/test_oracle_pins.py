@@ -1286,3 +1286,58 @@ def test_fixed_algorithm_cube_root_and_sech2_against_libm(O):
     assert np.max(np.abs(s - ref) / ref) <= 6 * np.finfo(float).eps
     assert O.sech2_fixed(0.0) == 1.0 and O.sech2_fixed(400.0) == 0.0
     assert O.sech2_fixed(1.3) == O.sech2_fixed(-1.3)
+
+
+# ---------------------------------------------------------------- R32: start vector of the solve
+def test_start_vector_is_the_quadratic_extrapolation_of_the_solution_increments(O):
+    # R32: x0 = s1 + 3 (s2 - s3) - 3 (s4 - s5) + (s6 - s7) once seven solutions exist since the last
+    # set_state (s1 the most recent), the plain previous solution before that.  Transcribed here from
+    # the recorded solutions of nine successive solves; polynomial exactness: the formula reproduces
+    # a sequence whose same-kind increments i_k = s_k - s_(k-1) are quadratic in k.
+    st = inputs.random_smooth_state(40, 28, 0.3, 0.2, seed=9, depth=1.0, rough=0.3)
+    o = O.Oracle(40, 28, 0.3, 0.2, st["H"], bc_xlo=PER, bc_xhi=PER, bc_ylo=WALL, bc_yhi=OUT)
+    o.set_state(st["h"], st["qx"], st["qy"], st["w"], st["p"])
+    assert np.array_equal(o.start_vector()[:, :-1], st["p"][:, :-1])   # no history yet: the state's p
+    sols = []
+    for k in range(9):
+        o.nonhydro_correct(0.01 * (1.0 + 0.1 * k))           # one solve each, on an evolving state
+        sols.append(o.get_state()["p"].copy())
+        x0 = o.start_vector()
+        if len(sols) < 7:
+            assert np.array_equal(x0[:, :-1], sols[-1][:, :-1])   # (periodic duplicate column aside)
+        else:
+            s = sols[::-1]
+            ref = ((s[0] + 3.0 * (s[1] - s[2])) - 3.0 * (s[3] - s[4])) + (s[5] - s[6])
+            assert np.array_equal(x0[:, :-1], ref[:, :-1])
+    # exactness on a synthetic sequence: increments of alternating kind, each kind quadratic in time
+    k = np.arange(9.0)
+    inc = np.where(k % 2 == 0, 1.0 + 0.3 * k + 0.05 * k * k, -0.2 + 0.1 * k - 0.02 * k * k)
+    seq = np.cumsum(inc)
+    pred = seq[7] + 3 * (seq[6] - seq[5]) - 3 * (seq[4] - seq[3]) + (seq[2] - seq[1])
+    assert pred == pytest.approx(seq[8], rel=1e-13)
+    # a new state forgets the history
+    o.set_state(st["h"], st["qx"], st["qy"], st["w"], st["p"])
+    assert np.array_equal(o.start_vector()[:, :-1], st["p"][:, :-1])
+
+
+def test_start_vector_changes_the_iteration_count_not_the_result(O):
+    cfg = inputs.make_config(3, nx=96, ny=96)
+    out = {}
+    for ws in (0, 1):
+        o = make(O, cfg, warm_start=ws)
+        o.step(3)                                   # six solves: no extrapolation yet in either run
+        first = o.get_state()
+        i3 = o.info().iters_total
+        o.step(27)
+        out[ws] = (first, i3, o.get_state(), o.info().iters_total - i3)
+    for k in ("h", "qx", "qy", "w", "p"):
+        assert np.array_equal(out[0][0][k], out[1][0][k])      # identical until seven solutions exist
+    assert out[0][1] == out[1][1]
+    assert out[1][3] < 0.85 * out[0][3]                        # ... then >= 15 % fewer iterations
+    h0, g = cfg["h0"], 9.81
+    c0 = np.sqrt(g * h0)
+    a, b = out[0][2], out[1][2]
+    assert np.max(np.abs(a["h"] - b["h"])) <= 1e-9 * h0        # same result at the north_star bars
+    qs = max(np.max(np.abs(a["qx"])), np.max(np.abs(a["qy"])), 1e-3 * h0 * c0)
+    assert max(np.max(np.abs(a["qx"] - b["qx"])), np.max(np.abs(a["qy"] - b["qy"]))) <= 1e-9 * qs
+    assert np.max(np.abs(a["p"] - b["p"])) <= 1e-9 * max(np.max(np.abs(a["p"])), 1e-3 * g * h0)
