@@ -17,6 +17,13 @@ time; no data-path collective.
 
 --impl reference: the CPU oracle (oracle/, as it stands) timed on the host cores on a bounded
 crop of the same workload (rank 0 only).
+
+Other modes (records for profiles/, not the driver's line): --solver srj (the paper's own solver),
+--precision 32 (the labelled fp32 variant), --hydrostatic (SWE mode: alu-bound predictor roofline
+against the fp64 rate measured live), --onesolve (one isolated solve for the ncu capture behind
+profiles/traffic.json), --table2 (the paper's timing experiment), --fullruns (every config at full
+size and length), --parityruns [--spread] [--solver srj] [--precision 32] [--param k=v] (the CUDA
+path beside the oracle over a configured horizon, ratios at the parity bars every 10 %).
 """
 import argparse
 import json
@@ -633,7 +640,7 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=5)   # >= 4 steps fill the start-vector history (R32)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", type=int, default=5)
     ap.add_argument("--nx", type=int, default=0)

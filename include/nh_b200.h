@@ -128,7 +128,10 @@ void nh_destroy(nh_ctx* ctx);
 /* State = conserved variables (h, qx, qy) per cell (L45-59, L528) and (w, p) per staggered node
  * (L245-247, L464-466, L535).  w, p NULL => zeros.  set stages the arrays in a free slot,
  * validates h >= 0 and finiteness there on the device, waits for that result (one stream
- * synchronisation) and returns NH_EINVAL leaving the current state untouched if it fails.
+ * synchronisation) and returns NH_EINVAL leaving the current state untouched if it fails.  A p that
+ * is bit-identical to the most recent pressure solution marks a continuation of the running state
+ * (checkpoint, round trip through the host): the solver keeps its solution history (R32);
+ * any other p (or NULL) starts a new one.
  * get: NULL => skip that field; synchronises (the arrays are complete on return). */
 int nh_set_state(nh_ctx* ctx, const double* h, const double* qx, const double* qy,
                  const double* w, const double* p);

@@ -1112,7 +1112,14 @@ int nho_set_state(nho_ctx* c, const double* h, const double* qx, const double* q
   memcpy(c->qy, qy, nc * sizeof(double));
   nodes_in(c, w, c->w);
   nodes_in(c, p, c->p);
-  c->nhist = 0;   /* R32: the solution history belongs to the replaced state */
+  /* R32: a p bit-identical to the most recent solution marks a continuation of the running state (a
+   * checkpoint, a round trip through the caller): the solution history stays valid; any other p
+   * starts a new history */
+  int cont = (p != NULL) && c->nhist > 0;
+  for (int J = 0; cont && J < c->nny; ++J)
+    for (int I = 0; I < c->nnx; ++I)
+      if (c->p[NIDX(c, I, J)] != c->hist[0][NIDX(c, I, J)]) { cont = 0; break; }
+  if (!cont) c->nhist = 0;
   return NHO_OK;
 }
 

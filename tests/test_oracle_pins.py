@@ -1341,3 +1341,27 @@ def test_start_vector_changes_the_iteration_count_not_the_result(O):
     qs = max(np.max(np.abs(a["qx"])), np.max(np.abs(a["qy"])), 1e-3 * h0 * c0)
     assert max(np.max(np.abs(a["qx"] - b["qx"])), np.max(np.abs(a["qy"] - b["qy"]))) <= 1e-9 * qs
     assert np.max(np.abs(a["p"] - b["p"])) <= 1e-9 * max(np.max(np.abs(a["p"])), 1e-3 * g * h0)
+
+
+def test_set_state_keeps_the_solution_history_only_for_a_continuation(O):
+    # R32: handing back the running state (p bit-identical to the most recent solution) keeps the
+    # history -- the run continues exactly as if set_state had not been called; any other p resets it
+    cfg = inputs.make_config(3, nx=64, ny=64)
+    a, b = make(O, cfg), make(O, cfg)
+    a.step(6)
+    b.step(6)
+    s = b.get_state()
+    b.set_state(s["h"], s["qx"], s["qy"], s["w"], s["p"])                 # round trip
+    assert np.max(np.abs(b.start_vector() - s["p"])) > 0.0                # still extrapolating
+    a.step(3)
+    b.step(3)
+    sa, sb = a.get_state(), b.get_state()
+    for k in sa:
+        assert np.array_equal(sa[k], sb[k]), k
+    assert a.info().iters_total == b.info().iters_total
+    p2 = s["p"].copy()
+    p2[5, 7] += 1e-9
+    b.set_state(s["h"], s["qx"], s["qy"], s["w"], p2)                     # a different p: new history
+    assert np.array_equal(b.start_vector(), p2)
+    b.set_state(s["h"], s["qx"], s["qy"], s["w"], None)
+    assert np.all(b.start_vector() == 0.0)
