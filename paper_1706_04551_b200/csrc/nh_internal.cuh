@@ -221,7 +221,7 @@ struct Ctx {
   int nhist;      // how many of them are valid (reset by set_state)
   real* p;   // pressure multiplier p~ (warm start of the next solve)
   real* b;   // right-hand side
-  real *dg, *dinv, *cE, *cW, *cN, *cS;  // diag(A), its inverse, column-scaled off-diagonals
+  real *dg, *dinv, *cE, *cW, *cN, *cS;  // diag(A), its inverse, off-diagonals (solver 1: row-scaled; hooks: raw)
   real *ky, *kr, *krB, *kr0, *kpA, *kpB, *kvA, *kvB, *kt;  // BiCGStab vectors (r, p, v double-buffered)
   double* pub;   // dense (nx+1) x (ny+1) staging plane for the public node layout
   std::vector<void*> raw;  // allocation bases (node planes are handed out offset to node (0,0))
@@ -265,7 +265,6 @@ void nh_launch_breaking(Ctx* c, const real* h, const real* qx1, const real* qy1,
 void nh_launch_rhs(Ctx* c, const real* h, const real* qx, const real* qy, const real* z,
                    const real* w, real* b, int constraint_only);
 void nh_launch_coeffs(Ctx* c, const real* h, const real* z);  // -> dg, dinv, raw cE..cS
-void nh_launch_scale_coeffs(Ctx* c);  // solver 0: cX *= dinv(neighbour)
 void nh_launch_scale_rows(Ctx* c, const real* b, real* bp);
 void nh_launch_assemble_rows(Ctx* c, const real* h, const real* qx, const real* qy,
                              const real* z, const real* w, real* bp);  // solver 1: rhs + rows + scaling fused  // solver 1: cX *= dinv, bp = b dinv, rho, max|bp|

@@ -1,7 +1,8 @@
 // nh_pressure.cu -- second and third parts of the time step, outside the Krylov loop:
-// breaking sources (a4), right-hand side (a5), the rows of the compact finite-difference pressure
-// operator (S8) and their column scaling for the Jacobi-preconditioned solver, the matrix-free
-// operator apply (test hook), the Chorin-Temam correction (a7) and the relaxation zone (a9).
+// breaking sources (a4), right-hand side (a5), the cell planes of the matrix-free solver, the rows
+// of the compact finite-difference pressure operator (S8: solver 1 and the test hooks), the
+// matrix-free operator apply (test hook), the w transport (R30), the start vector (R32), the
+// Chorin-Temam correction (a7) and the relaxation zones (a9).
 //
 // These kernels run once per Runge-Kutta stage (the solver runs 10^2 iterations per stage), so
 // they read their small stencils straight from global memory through the boundary index maps
@@ -143,21 +144,6 @@ k_coeffs(NhGrid G, const real* __restrict__ h, const real* __restrict__ z,
   size_t k = (size_t)J * G.np + I;
   dg[k] = AC; dinv[k] = RC(1.0) / AC;
   cE[k] = AE; cW[k] = AW; cN[k] = AN; cS[k] = AS;
-}
-
-// Column scaling for the right-preconditioned operator A M^-1, M = diag(A_C) (R14):
-// (A M^-1)_{n,nb} = A_{n,nb} / A_C(nb); its diagonal is 1.
-__global__ void __launch_bounds__(BX* BY)
-k_scale_coeffs(NhGrid G, const real* __restrict__ dinv, real* __restrict__ cE,
-               real* __restrict__ cW, real* __restrict__ cN, real* __restrict__ cS) {
-  int I = blockIdx.x * BX + threadIdx.x, J = blockIdx.y * BY + threadIdx.y;
-  if (I >= G.nnx || J >= G.nny) return;
-  Fld F{G, node_interior(G, I, J)};
-  size_t k = (size_t)J * G.np + I;
-  cE[k] = cE[k] * F.node(dinv, I + 1, J);
-  cW[k] = cW[k] * F.node(dinv, I - 1, J);
-  cN[k] = cN[k] * F.node(dinv, I, J + 1);
-  cS[k] = cS[k] * F.node(dinv, I, J - 1);
 }
 
 // Row scaling for solver 1 (the paper's Jacobi method, R28): c_X = A_X / A_C, b' = b / A_C; the
@@ -600,11 +586,6 @@ void nh_launch_rhs(Ctx* c, const real* h, const real* qx, const real* qy, const 
 void nh_launch_coeffs(Ctx* c, const real* h, const real* z) {
   k_coeffs<<<grid2(c->g.nnx, c->g.nny), dim3(BX, BY), 0, c->stream>>>(c->g, h, z, c->dg, c->dinv,
                                                                      c->cE, c->cW, c->cN, c->cS);
-  c->launches++;
-}
-void nh_launch_scale_coeffs(Ctx* c) {
-  k_scale_coeffs<<<grid2(c->g.nnx, c->g.nny), dim3(BX, BY), 0, c->stream>>>(c->g, c->dinv, c->cE,
-                                                                           c->cW, c->cN, c->cS);
   c->launches++;
 }
 void nh_launch_scale_rows(Ctx* c, const real* b, real* bp) {
