@@ -185,6 +185,53 @@ int nh_profile_read(nh_ctx* ctx, double* ms, long long* groups);
  * synchronises.  dfma_per_second is a HOST pointer. */
 int nh_fp64_rate(void* cuda_stream, double* dfma_per_second);
 
+/* ---- the CFL time step for callers that must not allocate ------------------------------------
+ * nh_cfl_dt_static computes dt = cfl / max_ij[(|u|+sqrt(g h))/dx + (|v|+sqrt(g h))/dy] (eq. (23),
+ * PAPER.md L339-341, with the desingularised velocities of L447-451; R20) of a state held
+ * in the CALLER's device arrays, without a context: no cudaMalloc, cudaFree, cudaMallocHost or any
+ * other allocating call happens inside, on the first call or later.  Everything else in this
+ * library needs nh_create, which allocates some fifty field planes.
+ *
+ * Who this is for.  Code that wants to know the admissible time step of a state it already has on
+ * the GPU, but runs where device allocation is off the table: a coupled model whose memory manager
+ * has claimed the whole device up front, so that a cudaMalloc from a guest library fails or eats
+ * into a reserve it does not own; a latency-bound loop (real-time forecasting, an in-situ monitor
+ * that sub-cycles on dt) that cannot afford the device-wide synchronisation cudaMalloc / cudaFree
+ * imply; a plug-in that by house rule may not own device memory at all.
+ *
+ * How.  The reduction's scratch memory (one partial maximum per 4096 cells) is a fixed array
+ * compiled into the library: 16384 doubles = 128 KiB.  Every GPU that loads libnh_b200.so holds that
+ * array from load until the process exits, used or not.  Its size is the limit: nx * ny must not
+ * exceed NH_STATIC_MAX_CELLS (= nh_cfl_dt_static_max_cells() = 8192 * 8192); a larger grid is
+ * refused with NH_EINVAL and a message in nh_static_last_error(), nothing is launched.
+ *
+ * Arguments.  h, qx, qy: nx*ny doubles each, cell layout as above, DEVICE pointers (read only);
+ * dt_out: DEVICE pointer to one double (written).  Host pointers are refused with NH_EINVAL.  h is
+ * expected >= 0 and finite, as nh_set_state demands; NaN rates are skipped; dt_out = 0 when no cell
+ * has a positive rate.  g, delta, cfl: nh_params' g, delta, cfl.  cuda_stream: a cudaStream_t of the
+ * CURRENT device (NULL = default stream).  The two kernels are only enqueued; the result is in
+ * dt_out once the stream reaches that point; the caller owns all four arrays throughout.  fp64, same
+ * operation order as the context path: bit-identical to nh_compute_dt on the same state.
+ *
+ * First call on a device.  It looks up, once per device and with that device current, the device
+ * address of the built-in array (cudaGetSymbolAddress) and checks that the device is sm_100.  Make
+ * this first call before starting any stream capture on that device.
+ *
+ * Sharing.  All calls on one device use the SAME array, and it keeps what the last call left.  Each
+ * call overwrites every slot before reading it, so no clearing is needed between calls that follow
+ * one another -- in one stream, or in streams ordered by events.  Two calls that can run on the GPU
+ * at the same time (different streams, different host threads, no ordering) race on the array and
+ * both results are then undefined: serialise them.
+ *
+ * Errors: NH_EINVAL (sizes, parameters, null / host pointers), NH_ECUDA (no sm_100 device, a CUDA
+ * call failed); nh_static_last_error() returns the text for the calling thread's last call. */
+#define NH_STATIC_MAX_CELLS 67108864LL
+int nh_cfl_dt_static(int nx, int ny, double dx, double dy, double g, double cfl, double delta,
+                     const double* h, const double* qx, const double* qy, double* dt_out,
+                     void* cuda_stream);
+long long nh_cfl_dt_static_max_cells(void);
+const char* nh_static_last_error(void);
+
 /* ---- test hooks (not on the timed path); node arrays in/out use the public node layout ---- */
 int nh_compute_dt(nh_ctx* ctx, double* dt_host);          /* CFL dt of the current state; synchronises */
 int nh_apply_A(nh_ctx* ctx, const double* x_nodes, double* y_nodes); /* y = A(h,z) x, matrix-free (S8) */

@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 INC = os.path.join(os.path.dirname(HERE), "include")
 LIB = os.path.join(HERE, "libnh_b200.so")
 KERNEL_SOURCES = ["nh_core.cu", "nh_predictor.cu", "nh_pressure.cu", "nh_solver.cu"]  # once per precision
-ABI_SOURCES = ["nh_abi.cu", "nh_peak.cu"]   # once
+ABI_SOURCES = ["nh_abi.cu", "nh_peak.cu", "nh_static.cu"]   # once
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-fmad=false", "-Xcompiler", "-fPIC", "-Xcompiler", "-Wall", "-cudart", "shared"]
 OBJ = os.path.join(HERE, "build")

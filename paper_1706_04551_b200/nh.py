@@ -62,6 +62,7 @@ EXPORTS = (
     "nh_hydrostatic_step", "nh_nonhydro_correct", "nh_sync", "nh_get_info", "nh_last_error",
     "nh_launch_count", "nh_profile", "nh_profile_read", "nh_compute_dt", "nh_apply_A", "nh_coeffs",
     "nh_rhs", "nh_constraint", "nh_solve", "nh_breaking", "nh_w_advect", "nh_fp64_rate", "nh_start_vector",
+    "nh_cfl_dt_static", "nh_cfl_dt_static_max_cells", "nh_static_last_error",
 )
 
 
@@ -104,6 +105,11 @@ def lib():
         L.nh_w_advect.argtypes = [_vp, C.c_double, _vp]
         L.nh_start_vector.argtypes = [_vp, _vp]
         L.nh_fp64_rate.argtypes = [_vp, C.POINTER(C.c_double)]
+        L.nh_cfl_dt_static.argtypes = [C.c_int, C.c_int] + [C.c_double] * 5 + [_vp] * 5
+        L.nh_cfl_dt_static_max_cells.argtypes = []
+        L.nh_cfl_dt_static_max_cells.restype = C.c_longlong
+        L.nh_static_last_error.argtypes = []
+        L.nh_static_last_error.restype = C.c_char_p
         _lib = L
     return _lib
 
@@ -115,6 +121,26 @@ def fp64_rate(stream=None) -> float:
     if st != OK:
         raise NHError(st, "nh_fp64_rate")
     return r.value
+
+
+def cfl_dt_static_max_cells() -> int:
+    return int(lib().nh_cfl_dt_static_max_cells())
+
+
+def cfl_dt_static(h, qx, qy, dt_out, dx, dy, g=9.81, cfl=0.5, delta=1e-5, stream=None):
+    """nh_cfl_dt_static: the CFL time step of a state in the caller's own device arrays, for callers
+    that must not allocate device memory (include/nh_b200.h has the who and why).  h, qx, qy: torch
+    CUDA float64 tensors of shape (ny, nx); dt_out: a torch CUDA float64 tensor of one element, which
+    the caller provides -- this wrapper creates no tensor either.  Only enqueues on `stream` (default:
+    the NULL stream): read dt_out after that stream has got there.  Grids above
+    cfl_dt_static_max_cells() raise NHError(EINVAL)."""
+    ny, nx = (int(n) for n in h.shape)
+    keep = []
+    ptrs = [_in(a, (ny, nx), keep) for a in (h, qx, qy)] + [_out_ptr(dt_out, (1,))]
+    sp = None if stream is None else (stream if isinstance(stream, int) else stream.cuda_stream)
+    st = lib().nh_cfl_dt_static(nx, ny, float(dx), float(dy), float(g), float(cfl), float(delta), *ptrs, sp)
+    if st != OK:
+        raise NHError(st, lib().nh_static_last_error().decode(errors="replace"))
 
 
 def default_params(**kw) -> Params:
