@@ -284,15 +284,18 @@ def run_b200(args):
     # ---- roofline of the dominant kernel (the BiCGStab solve), timed live with CUDA events
     peak, peak_src = _peaks()
     sol_ms, sol_n = prof["solver"]
-    node_iters = (iters + solves) * float(nn)          # + the polish iteration of every solve
-    bytes_unit = BYTES_PER_NODE_ITER * (0.5 if args.precision == 32 else 1.0)
-    if args.solver == "srj":   # one Jacobi sweep: reads x, b', 4 coefficients, writes x'
-        bytes_unit = 56.0 * (0.5 if args.precision == 32 else 1.0)
-        node_iters = (iters + solves) * float(nn)      # + the sweep that meets the stopping rule
-    achieved = bytes_unit * node_iters / (sol_ms * 1e-3) / 1e9 if sol_ms > 0 else 0.0
-    # bytes this kernel itself must move per node-iteration: the matrix-free two-pass
-    # iteration reads / writes 18 planes (144 B in fp64) -- SURVEY 8(d)'s "lower bound"; k_srj: 7 planes.
-    kernel_unit = (56.0 if args.solver == "srj" else 144.0) * (0.5 if args.precision == 32 else 1.0)
+    node_iters = (iters + solves) * float(nn)          # + the polish iteration of every solve (solver 1: + the
+                                                       # sweep that meets the stopping rule)
+    half = 0.5 if args.precision == 32 else 1.0
+    # ALGORITHMIC bytes per node-iteration of the kernel as built: the matrix-free
+    # two-pass BiCGStab iteration reads / writes 18 planes (144 B in fp64); one Jacobi sweep of k_srj reads
+    # x, b', 4 coefficients and writes x' (56 B).  `achieved` and `frac` are computed from THIS figure.
+    # SURVEY 8(d)'s 160 B describes a solver with stored rows; the rate on that model is only the labelled
+    # side field `effective_on_survey_160B_model` (it overstates the DRAM rate of this kernel by 11 %).
+    bytes_unit = (56.0 if args.solver == "srj" else 144.0) * half
+    survey_unit = (56.0 if args.solver == "srj" else BYTES_PER_NODE_ITER) * half
+    per_s = node_iters / (sol_ms * 1e-3) / 1e9 if sol_ms > 0 else 0.0
+    achieved = bytes_unit * per_s
     # measured DRAM traffic: ncu dram__bytes_read + write per node-iteration of the SAME kernel
     # (profiles/traffic.json names the capture), scaled by this run's node-iterations per launch
     traffic, traffic_unit = None, None
@@ -314,9 +317,14 @@ def run_b200(args):
                                   " (one cooperative launch per pressure solve)",
         "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": traffic,
         "peak_source": peak_src, "frac_of_nominal_8TBs": achieved / 8000.0,
-        "bytes_per_node_iteration": bytes_unit, "bytes_source": "SURVEY.md 8(d) per-unit figure (fp32 variant: half)",
-        "kernel_bytes_per_node_iteration": kernel_unit,
-        "frac_of_kernel_bytes": (kernel_unit / bytes_unit) * achieved / peak,
+        "bytes_per_node_iteration": bytes_unit,
+        "bytes_source": "the planes this kernel must move per node-iteration (DESIGN.md section 6; fp32 variant: half)",
+        "effective_on_survey_160B_model": {"bytes_per_node_iteration": survey_unit, "GB/s": survey_unit * per_s,
+                                           "frac": survey_unit * per_s / peak,
+                                           "note": "SURVEY.md 8(d) per-unit figure of a stored-row solver: not this "
+                                                   "kernel's DRAM rate"},
+        "achieved_dram": {"GB/s": traffic_unit * per_s, "frac": traffic_unit * per_s / peak}
+                         if traffic_unit is not None else None,
         "traffic_per_node_iteration": traffic_unit,
         "traffic_note": "derived: ncu DRAM bytes per node-iteration of this kernel (profiles/traffic.json) x this run's "
                         "node-iterations per launch" if traffic is not None else None,
