@@ -4,7 +4,8 @@ same seeded inputs (-m gpu; needs a B200).
 Bars (BASELINE.json north_star; SURVEY.md 8(d) "Parity metric"):
   * after whole steps:  max|eta_gpu - eta_orc| <= 1e-9 h0;  for a in (qx, qy, w, p):
     max|a_gpu - a_orc| <= 1e-9 max(max|a_orc|, floor_a),
-    floor = 1e-3 (h0 c0, h0 c0, c0, g h0), c0 = sqrt(g h0);
+    floor = 1e-3 (h0 c0, h0 c0, c0, g h0), c0 = sqrt(g h0) -- per field, qx and qy each on its own;
+    the weaker joint bar on the discharge vector is used only where a test passes vector_bar=True;
   * everything outside the Krylov solver (predictor, coefficients, right-hand side, constraint,
     operator apply, CFL dt) is evaluated in the same IEEE fp64 operation order on both sides
     (-fmad=false / -ffp-contract=off), so those are compared BIT-EXACTLY;
@@ -47,26 +48,32 @@ def rnd_cfg(nx, ny, bcs, seed, dry=0.0, dx=0.5, dy=0.4, depth=1.0, **prm):
 
 
 def parity(go, oo, H, h0, g=9.81, tol=1e-9):
-    """-> dict of (error / allowed) ratios; all must be <= 1.  north_star bars:
-    max|d eta| <= tol h0; relative L-infinity <= tol on the discharge, w and p, with floors 1e-3 of
-    the natural scales.  The discharge q = (qx, qy) is ONE vector field: both components are judged
-    against max|q| (a bar per component would depend on the orientation of the axes -- a wave along
-    x has qy ~ 0 -- while the admissible solver error, any p~ with residual <= 1e-12 (R23), enters
-    both components alike through dt h grad p~)."""
+    """-> dict of (error / allowed) ratios.  north_star bars:
+    max|d eta| <= tol h0; relative L-infinity <= tol on qx, qy, w and p, each against its OWN maximum
+    with a floor of 1e-3 of the natural scale: keys eta, qx_own, qy_own, w, p.  Beside them, keys qx
+    and qy judge the discharge as ONE vector field against max|q|: a weaker bar (a wave along x has
+    qy ~ 0, while the admissible solver error -- any p~ with residual <= 1e-12, R23 -- enters both
+    components alike through dt h grad p~), used only where a test says so and DESIGN.md section 4
+    lists it."""
     c0 = np.sqrt(g * h0)
     out = {}
     out["eta"] = np.max(np.abs((go["h"] - H) - (oo["h"] - H))) / (tol * h0)
     qscale = max(np.max(np.abs(oo["qx"])), np.max(np.abs(oo["qy"])), 1e-3 * h0 * c0)
     for k in ("qx", "qy"):
         out[k] = np.max(np.abs(go[k] - oo[k])) / (tol * qscale)
+        out[k + "_own"] = np.max(np.abs(go[k] - oo[k])) / (tol * max(np.max(np.abs(oo[k])), 1e-3 * h0 * c0))
     for k, f in dict(w=c0, p=g * h0).items():
         scale = max(np.max(np.abs(oo[k])), 1e-3 * f)
         out[k] = np.max(np.abs(go[k] - oo[k])) / (tol * scale)
     return out
 
 
-def assert_parity(go, oo, H, h0, tol=1e-9):
+def assert_parity(go, oo, H, h0, tol=1e-9, vector_bar=False):
+    """All ratios <= 1, the per-component discharge bars included.  vector_bar=True (a deviation from
+    north_star, each use listed in DESIGN.md section 4) drops qx_own / qy_own and keeps the joint bar."""
     r = parity(go, oo, H, h0, tol=tol)
+    if vector_bar:
+        r = {k: v for k, v in r.items() if not k.endswith("_own")}
     assert all(np.isfinite(v) and v <= 1.0 for v in r.values()), r
 
 
@@ -258,16 +265,38 @@ def test_config4_beach_reduced(O, G):
     # The full horizon is compared bit for bit under solver 1 (tests/test_gpu_horizon.py).
     cfg = inputs.make_config(4, nx=640, ny=8)
     o, g = both(O, G, cfg)
+    # vector_bar: the strip is 8 cells wide and the wave runs along x, so max|qy| is four orders below
+    # max|qx| while the solver-level difference enters both components alike; qy alone against its own
+    # maximum misses 1e-9 here (the only test of the suite that does: DESIGN.md section 4).
     for n in (150, 30, 30):
         o.step(n)
         g.step(n)
         assert g.sync() == 0
-        assert_parity(g.get_state(), o.get_state(), cfg["H"], cfg["h0"])
+        assert_parity(g.get_state(), o.get_state(), cfg["H"], cfg["h0"], vector_bar=True)
     # Clamps here are round-off events (|h*| ~ 1e-17 < 0 in dry shoreline cells, driven by the
     # 1e-12-level solver noise that the elliptic solve spreads to the still shoreline), so their
     # count is not unique across two valid solves (R7/R23): compare the state (above),
     # and check that both sides see the same kind of event.
     assert (g.info().clamps > 0) == (o.info().clamps > 0)
+
+
+@pytest.mark.xfail(strict=False, reason="known limit: config 4 with the default BiCGStab solver misses the 1e-9 bars "
+                   "outside the quiet window (two oracle runs at rtol 1e-12 / 1e-13 differ as much: profiles/r02b); "
+                   "the bars are met bit for bit under solver 1 (tests/test_gpu_horizon.py)")
+def test_config4_beach_reduced_at_the_original_checkpoints_known_limit(O, G):
+    # the checkpoints this comparison had before the sensitivity was measured (steps 100, 200, 300), kept so
+    # that the miss stays on record: north_star's "within 1e-9 on all five configs" does NOT hold for config 4
+    # with solver 0 at these steps (README).  The failure message carries the ratios.
+    cfg = inputs.make_config(4, nx=640, ny=8)
+    o, g = both(O, G, cfg)
+    seen = {}
+    for n in (100, 100, 100):
+        o.step(n)
+        g.step(n)
+        assert g.sync() == 0
+        r = parity(g.get_state(), o.get_state(), cfg["H"], cfg["h0"])
+        seen[int(g.info().steps)] = {k: float("%.3g" % v) for k, v in r.items()}
+    assert all(v <= 1.0 for r in seen.values() for v in r.values()), seen
 
 
 def test_config5_tsunami_crops(O, G):
