@@ -107,11 +107,16 @@ typedef struct {
   long long solves;
   int iters_last, iters_max;
   int flags;             /* bit0: a solve failed to converge; bit1: NaN/Inf dt or rhs;
-                            bit2: the last set_state saw h<0 or a non-finite value (rejected) */
+                            bit2: the last set_state saw h<0 or a non-finite value (rejected);
+                            bit3 (fp32 variant only, informational, sticky, no error code): a solve was
+                            accepted because its true residual stopped improving ABOVE
+                            solver_rtol_effective -- look at res_last                         */
   int reserved;
   double clamp_max;      /* largest |h*| of a clamped negative depth (R7, R24)             */
   long long clamp_hist[6]; /* clamps by size of |h*| in metres: < 1e-15, < 1e-12, < 1e-9, < 1e-6,
                             < 1e-3, >= 1e-3                                                 */
+  double solver_rtol_effective; /* the tolerance solver 0 really stops at: nh_params.solver_rtol, except
+                            that the fp32 variant raises anything below 1e-4 to 1e-4            */
 } nh_info;
 
 void nh_default_params(nh_params* prm);
@@ -137,8 +142,20 @@ int nh_set_state(nh_ctx* ctx, const double* h, const double* qx, const double* q
                  const double* w, const double* p);
 int nh_get_state(nh_ctx* ctx, double* h, double* qx, double* qy, double* w, double* p);
 /* Simulated time of the current state (default 0 at nh_create).  Together with nh_get_state /
- * nh_set_state and nh_get_info().t this is the checkpoint / restart: the generating relaxation zone
- * (L417-431) is the only part of the step that reads the clock.  Enqueued on the stream. */
+ * nh_set_state and nh_get_info().t this is the checkpoint / restart of the FIELDS: the generating
+ * relaxation zone (L417-431) is the only part of the step that reads the clock.  Enqueued on the stream.
+ * Two pieces of state are NOT in that checkpoint and stay inside the context:
+ *  (1) the onset / termination flags of the breaking criterion (eq. (9)).  They survive
+ *      nh_set_state and start cleared in a new context.  With B1 < B2 (the default 0.15 / 0.5) the
+ *      criterion does not consult them, so a restart in a fresh context is equivalent; with B1 >= B2
+ *      (true hysteresis) it is not, and there is no call to export them.
+ *  (2) the solver's history of the last seven pressure solutions (start vector, R32).  It is
+ *      kept only when the p given to nh_set_state is bit-identical to the last solution AS SOLVED; a
+ *      generating or absorbing relaxation zone modifies p after the solve, so with gen_on or abs_* > 0
+ *      every get-then-set round trip starts a new history (seven solves from the previous solution
+ *      alone: more iterations, same converged result).  A fresh context always starts a new one.
+ * Neither changes what a converged step computes beyond the solver tolerance, except (1) with
+ * B1 >= B2. */
 int nh_set_time(nh_ctx* ctx, double t);
 
 /* nsteps full time steps: dt = CFL / max[(|u|+sqrt(gh))/dx + (|v|+sqrt(gh))/dy] (eq. (23),

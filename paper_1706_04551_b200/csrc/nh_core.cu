@@ -564,6 +564,7 @@ int core_get_info(Ctx* c, nh_info* out) {
   out->flags = s.flags;
   memcpy(&out->clamp_max, &s.clamp_max_bits, sizeof(double));
   for (int k = 0; k < 6; ++k) out->clamp_hist[k] = (long long)s.clamp_hist[k];
+  out->solver_rtol_effective = c->prm.solver_rtol;  // fp32 variant: raised to 1e-4 at create
   return NH_OK;
 }
 
@@ -702,7 +703,7 @@ int core_solve(Ctx* c, const double* b_nodes, double* x_nodes, int* iters, doubl
   if (relres) *relres = c->sc_host->res_last;
   int fl = c->sc_host->flags;
   // the hook reports its own solve; clear the sticky bits it may have set
-  k_clear_flag<<<1, 1, 0, c->stream>>>(c->sc, NH_FLAG_NOCONV | NH_FLAG_NAN);
+  k_clear_flag<<<1, 1, 0, c->stream>>>(c->sc, NH_FLAG_NOCONV | NH_FLAG_NAN | NH_FLAG_STAGNATED);
   c->launches++;
   if (fl & NH_FLAG_NAN) return NH_ENAN;
   if (fl & NH_FLAG_NOCONV) return NH_ENOCONV;

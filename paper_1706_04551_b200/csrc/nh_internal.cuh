@@ -65,7 +65,7 @@ struct NhScal {
   unsigned long long clamp_hist[6];   // < 1e-15, < 1e-12, < 1e-9, < 1e-6, < 1e-3, >= 1e-3 (metres)
 };
 
-enum { NH_FLAG_NOCONV = 1, NH_FLAG_NAN = 2, NH_FLAG_BADSTATE = 4 };
+enum { NH_FLAG_NOCONV = 1, NH_FLAG_NAN = 2, NH_FLAG_BADSTATE = 4, NH_FLAG_STAGNATED = 8 };
 #endif  // NH_SHARED_TYPES
 
 namespace NH_NS {

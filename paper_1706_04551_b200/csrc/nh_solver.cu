@@ -529,7 +529,7 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
     t = vC; vC = vN; vN = t;
   };
   int buf = 0;  // partial buffer of the pass in flight (alternates: one grid barrier per pass)
-  int iters = 0, converged = 0, status = 0;
+  int iters = 0, converged = 0, status = 0, stagnated = 0;
   double rnorm = 0.0, bnorm = 0.0, tol = 0.0, rnorm_prev = 0.0;
 
   phase_images(P);
@@ -551,8 +551,10 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
     if (rnorm <= tol) { converged = 1; break; }
     // fp32 variant: an fp32 iterate cannot satisfy the system better than ~ kappa u32 ||b||.  When a
     // whole cycle (recursive residual below tol) no longer halves the TRUE residual, the attainable
-    // accuracy has been reached: accept the iterate; res_last reports what was reached.
-    if (kEta && cycle > 0 && rnorm > 0.5 * rnorm_prev) { converged = 1; break; }
+    // accuracy has been reached: accept the iterate; res_last reports what was reached, and because
+    // that residual is ABOVE the tolerance the acceptance is flagged (NH_FLAG_STAGNATED, nh_info.flags
+    // bit 3): a breakdown that stalls at 1e-2 must not look like a solve that met 1e-4.
+    if (kEta && cycle > 0 && rnorm > 0.5 * rnorm_prev) { converged = 1; stagnated = 1; break; }
     rnorm_prev = rnorm;
     if (iters >= P.maxit) break;
     // first direction of the cycle: p = r, v = A M^-1 p, sigma = r0.v
@@ -623,6 +625,7 @@ __global__ void __launch_bounds__(NT, NH_MINB) k_bicgstab(SolveP P) {
     NhScal* sc = P.sc;
     if (status == NH_ENOCONV) sc->flags |= NH_FLAG_NOCONV;
     if (status == NH_ENAN) sc->flags |= NH_FLAG_NAN;
+    if (stagnated) sc->flags |= NH_FLAG_STAGNATED;
     sc->iters_last = iters;
     sc->res_last = (bnorm > 0.0) ? rnorm / bnorm : 0.0;
     if (P.count_stats) {

@@ -18,6 +18,7 @@ import numpy as np
 
 BC_PERIODIC, BC_WALL, BC_OUTFLOW = 0, 1, 2
 OK, EINVAL, ENOMEM, ECUDA, ENOCONV, ENAN = 0, -1, -2, -3, -4, -5
+FLAG_NOCONV, FLAG_NAN, FLAG_BADSTATE, FLAG_STAGNATED = 1, 2, 4, 8   # nh_info.flags
 PROF_CATS = ("predictor", "assembly", "solver", "correct")
 
 HERE = os.path.dirname(os.path.abspath(__file__))
@@ -45,6 +46,7 @@ class Info(C.Structure):
         ("solves", C.c_longlong),
         ("iters_last", C.c_int), ("iters_max", C.c_int), ("flags", C.c_int), ("reserved", C.c_int),
         ("clamp_max", C.c_double), ("clamp_hist", C.c_longlong * 6),
+        ("solver_rtol_effective", C.c_double),
     ]
 
 
