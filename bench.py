@@ -44,8 +44,8 @@ UNIT = "cell-updates/s"
 # Algorithmic bytes of the dominant kernel:
 # one Jacobi-preconditioned BiCGStab iteration moves >= 20 doubles per node.
 BYTES_PER_NODE_ITER = 160.0
-ORACLE_CROP = 640          # cpu_baseline / reference sample: crop of the config-5 basin (cells per side)
-ORACLE_STEPS = 5           # cpu_baseline leg: full RK2 steps timed on that crop (~10-30 s of host work)
+ORACLE_CROP = 640          # cpu_baseline / reference sample: crop of the config-5 basin (cells per side);
+                           # --oracle-crop changes it and the line says so (config.oracle_crop)
 
 
 def _peaks():
@@ -122,13 +122,13 @@ class ClockSampler:
         return out
 
 
-def _oracle_sample(steps, warmup, crop=None):
+def _oracle_sample(steps, warmup, crop):
     """Time the CPU oracle (as it stands) on a crop of the config-5 basin: same dx, depths,
-    conditioning (h/dx = 40); `steps` full RK2 NH steps after `warmup`."""
+    conditioning (h/dx = 40); `steps` full RK2 NH steps after `warmup`.  ONE protocol for the
+    cpu_baseline leg of the B200 arm and for `--impl reference`: both pass --steps / --warmup /
+    --oracle-crop as given, so the same flags time the same oracle work."""
     from oracle import nh_oracle
     from paper_1706_04551_b200 import inputs
-    if crop is None:   # NH_BENCH_ORACLE_CROP: smaller sample for the CPU test-suite only
-        crop = int(os.environ.get("NH_BENCH_ORACLE_CROP", ORACLE_CROP))
     cfg = inputs.make_config(5, nx=crop, ny=crop)
     o = nh_oracle.Oracle(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["H"], **cfg["params"])
     o.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
@@ -198,16 +198,17 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    r = _oracle_sample(args.steps, args.warmup)
+    r = _oracle_sample(args.steps, args.warmup, args.oracle_crop)
     line = {
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * r["seconds"] / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": "configs[4] tsunami 8192x8192 (timed on a bounded crop, see cpu_baseline.sample)",
-                   "solver": "Jacobi-BiCGStab rtol 1e-12", "iters_per_solve": r["iters_per_solve"]},
+                   "solver": "Jacobi-BiCGStab rtol 1e-12", "iters_per_solve": r["iters_per_solve"],
+                   "oracle_crop": args.oracle_crop},
         "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
-                         "sample": r["sample"]},
+                         "sample": r["sample"], "iters_per_solve": r["iters_per_solve"], "seconds": r["seconds"]},
         "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -335,28 +336,40 @@ def run_b200(args):
         "kernel_share_of_step": sol_ms / ms if ms > 0 else None,
       }
 
-    # ---- end-to-end leg: host buffers in and out through the C ABI every step
+    # ---- end-to-end leg: host buffers in and out through the C ABI every step, on the SAME step window as the
+    # device leg (steps W+1 .. W+K of the run): a fresh context is taken through the same warm-up -- its last
+    # warm-up step already through the host buffers (pages them in, same code path) -- so that both legs do
+    # the same solves (bit-identical states, same iteration counts) and differ only by the copies.  The state
+    # comes back through nh_continue_state: the caller says that the run goes on (the solver keeps its history).
+    sim.close()
+    sim = nh.NH(nx, ny, cfg["dx"], cfg["dy"], cfg["H"], stream=stream, **prm)
+    sim.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
     hb = [{k: torch.empty(cfg[k].shape, dtype=torch.float64).pin_memory() for k in ("h", "qx", "qy", "w", "p")}
           for _ in range(2)]
-    sim.get_state({k: v.numpy() for k, v in hb[0].items()})
-    for w_ in range(1):   # one untimed e2e step (page-in of the pinned buffers, same code path)
+
+    def e2e_step():
         a, b = hb[0], hb[1]
-        sim.set_state(*(a[k].numpy() for k in ("h", "qx", "qy", "w", "p")))
+        sim.set_state(*(a[k].numpy() for k in ("h", "qx", "qy", "w", "p")), keep_history=True)
         sim.step(1)
-        sim.get_state({k: v.numpy() for k, v in b.items()})
+        sim.get_state({k: v.numpy() for k, v in b.items()})   # synchronises: the result is on the host
         hb.reverse()
+
+    if args.warmup > 1:
+        sim.step(args.warmup - 1)
+    sim.get_state({k: v.numpy() for k, v in hb[0].items()})
+    if args.warmup >= 1:
+        e2e_step()
+    ie0 = sim.info()
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        a, b = hb[0], hb[1]
-        sim.set_state(*(a[k].numpy() for k in ("h", "qx", "qy", "w", "p")))
-        sim.step(1)
-        sim.get_state({k: v.numpy() for k, v in b.items()})   # synchronises: result is on the host
-        hb.reverse()
+        e2e_step()
     barrier()
     e2e_s = time.perf_counter() - t0
+    ie1 = sim.info()
     e2e_max = max_over_ranks(e2e_s, world, dev)
     e2e_value = whole_job_value(nc, args.steps, world, e2e_max)
+    e2e_iters = (ie1.iters_total - ie0.iters_total) / max(ie1.solves - ie0.solves, 1)
     st2 = sim.sync()
     io_bytes = 8 * (3 * nc + 2 * nn)
 
@@ -376,14 +389,17 @@ def run_b200(args):
                    "status": [int(st), int(st2)], "clamps": int(i1.clamps)},
         "clocks": clk,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": io_bytes,
-                "d2h_bytes_per_step": io_bytes, "ms_per_step": 1e3 * e2e_max / args.steps},
+                "d2h_bytes_per_step": io_bytes, "ms_per_step": 1e3 * e2e_max / args.steps,
+                "iters_per_solve": e2e_iters, "window": "steps %d..%d of the run, as the device leg" % (args.warmup + 1, args.warmup + args.steps)},
         "gpu_launches": int(launches),
         "roofline": roofline,
     }
     if rank == 0 and world == 1 and not args.no_cpu:
-        r = _oracle_sample(ORACLE_STEPS, 0)
+        r = _oracle_sample(args.steps, args.warmup, args.oracle_crop)   # what --impl reference runs on these flags
         line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
-                                "sample": r["sample"], "seconds": r["seconds"]}
+                                "sample": r["sample"], "seconds": r["seconds"],
+                                "iters_per_solve": r["iters_per_solve"]}
+        line["config"]["oracle_crop"] = args.oracle_crop
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
@@ -660,6 +676,8 @@ def main():
     ap.add_argument("--nx", type=int, default=0)
     ap.add_argument("--ny", type=int, default=0)
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--oracle-crop", type=int, default=ORACLE_CROP,
+                    help="cells per side of the config-5 crop the CPU oracle is timed on (cpu_baseline, --impl reference)")
     ap.add_argument("--precision", type=int, default=64, choices=[64, 32],
                     help="32: the optional fp32 variant (labelled as such; the fp64 line is the headline)")
     ap.add_argument("--solver", default="bicgstab", choices=["bicgstab", "srj"],

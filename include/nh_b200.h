@@ -133,13 +133,19 @@ void nh_destroy(nh_ctx* ctx);
 /* State = conserved variables (h, qx, qy) per cell (L45-59, L528) and (w, p) per staggered node
  * (L245-247, L464-466, L535).  w, p NULL => zeros.  set stages the arrays in a free slot,
  * validates h >= 0 and finiteness there on the device, waits for that result (one stream
- * synchronisation) and returns NH_EINVAL leaving the current state untouched if it fails.  A p that
- * is bit-identical to the most recent pressure solution marks a continuation of the running state
- * (checkpoint, round trip through the host): the solver keeps its solution history (R32);
- * any other p (or NULL) starts a new one.
+ * synchronisation) and returns NH_EINVAL leaving the current state untouched if it fails.
+ * nh_set_state starts a NEW run: the solver forgets its history of earlier pressure solutions
+ * (R32), so the next solves start from p alone.  nh_continue_state is the same call for a
+ * state that IS the running one coming back -- a checkpoint restored into the context that wrote it,
+ * a round trip through the host: the history is kept, and the run goes on exactly as if the state had
+ * never left (same iteration counts, same bits).  The caller says which it is; the library does not
+ * look at the contents to guess.  Handing nh_continue_state an unrelated state is not an error: the
+ * first solves merely start from a poor vector (more iterations, same converged result).
  * get: NULL => skip that field; synchronises (the arrays are complete on return). */
 int nh_set_state(nh_ctx* ctx, const double* h, const double* qx, const double* qy,
                  const double* w, const double* p);
+int nh_continue_state(nh_ctx* ctx, const double* h, const double* qx, const double* qy,
+                      const double* w, const double* p);
 int nh_get_state(nh_ctx* ctx, double* h, double* qx, double* qy, double* w, double* p);
 /* Simulated time of the current state (default 0 at nh_create).  Together with nh_get_state /
  * nh_set_state and nh_get_info().t this is the checkpoint / restart of the FIELDS: the generating
@@ -149,11 +155,9 @@ int nh_get_state(nh_ctx* ctx, double* h, double* qx, double* qy, double* w, doub
  *      nh_set_state and start cleared in a new context.  With B1 < B2 (the default 0.15 / 0.5) the
  *      criterion does not consult them, so a restart in a fresh context is equivalent; with B1 >= B2
  *      (true hysteresis) it is not, and there is no call to export them.
- *  (2) the solver's history of the last seven pressure solutions (start vector, R32).  It is
- *      kept only when the p given to nh_set_state is bit-identical to the last solution AS SOLVED; a
- *      generating or absorbing relaxation zone modifies p after the solve, so with gen_on or abs_* > 0
- *      every get-then-set round trip starts a new history (seven solves from the previous solution
- *      alone: more iterations, same converged result).  A fresh context always starts a new one.
+ *  (2) the solver's history of the last seven pressure solutions (start vector, R32).
+ *      nh_set_state drops it, nh_continue_state keeps it; a fresh context always starts without one
+ *      (seven solves from the previous solution alone: more iterations, same converged result).
  * Neither changes what a converged step computes beyond the solver tolerance, except (1) with
  * B1 >= B2. */
 int nh_set_time(nh_ctx* ctx, double t);

@@ -1098,8 +1098,8 @@ static void nodes_out(nho_ctx* c, const double* src, double* dst) {
     }
 }
 
-int nho_set_state(nho_ctx* c, const double* h, const double* qx, const double* qy,
-                  const double* w, const double* p) {
+static int set_state(nho_ctx* c, const double* h, const double* qx, const double* qy,
+                     const double* w, const double* p, int keep_history) {
   if (!c || !h || !qx || !qy) return NHO_EINVAL;
   size_t nc = (size_t)c->nx * (size_t)c->ny;
   for (size_t k = 0; k < nc; ++k)
@@ -1112,15 +1112,18 @@ int nho_set_state(nho_ctx* c, const double* h, const double* qx, const double* q
   memcpy(c->qy, qy, nc * sizeof(double));
   nodes_in(c, w, c->w);
   nodes_in(c, p, c->p);
-  /* R32: a p bit-identical to the most recent solution marks a continuation of the running state (a
-   * checkpoint, a round trip through the caller): the solution history stays valid; any other p
-   * starts a new history */
-  int cont = (p != NULL) && c->nhist > 0;
-  for (int J = 0; cont && J < c->nny; ++J)
-    for (int I = 0; I < c->nnx; ++I)
-      if (c->p[NIDX(c, I, J)] != c->hist[0][NIDX(c, I, J)]) { cont = 0; break; }
-  if (!cont) c->nhist = 0;
+  /* R32: set_state starts a new solution history; continue_state (the caller says that the running
+   * state is coming back: a checkpoint, a round trip) keeps it */
+  if (!keep_history) c->nhist = 0;
   return NHO_OK;
+}
+int nho_set_state(nho_ctx* c, const double* h, const double* qx, const double* qy,
+                  const double* w, const double* p) {
+  return set_state(c, h, qx, qy, w, p, 0);
+}
+int nho_continue_state(nho_ctx* c, const double* h, const double* qx, const double* qy,
+                       const double* w, const double* p) {
+  return set_state(c, h, qx, qy, w, p, 1);
 }
 
 int nho_get_state(nho_ctx* c, double* h, double* qx, double* qy, double* w, double* p) {

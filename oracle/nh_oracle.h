@@ -81,7 +81,11 @@ int  nho_create(nho_ctx** out, int nx, int ny, double dx, double dy, const doubl
                 const nho_params* prm);
 void nho_destroy(nho_ctx* c);
 int  nho_set_state(nho_ctx* c, const double* h, const double* qx, const double* qy,
-                   const double* w, const double* p);          /* w,p NULL => zeros     */
+                   const double* w, const double* p);          /* w,p NULL => zeros; a new run:
+                                                                  the solution history of R32 is dropped */
+int  nho_continue_state(nho_ctx* c, const double* h, const double* qx, const double* qy,
+                        const double* w, const double* p);     /* the same for the running state coming
+                                                                  back: the solution history is kept   */
 int  nho_get_state(nho_ctx* c, double* h, double* qx, double* qy, double* w, double* p); /* NULL => skip */
 int  nho_set_time(nho_ctx* c, double t);          /* simulated time of the current state (restart) */
 int  nho_step(nho_ctx* c, int nsteps);            /* CFL dt each step, RK per time_order */

@@ -51,6 +51,7 @@ def lib():
         L.nho_destroy.argtypes = [C.c_void_p]
         L.nho_destroy.restype = None
         L.nho_set_state.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp]
+        L.nho_continue_state.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp]
         L.nho_get_state.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, _dp]
         L.nho_set_time.argtypes = [C.c_void_p, C.c_double]
         L.nho_step.argtypes = [C.c_void_p, C.c_int]
@@ -137,10 +138,11 @@ class Oracle:
             raise OracleError(st, lib().nho_last_error(self._h).decode())
         return st
 
-    def set_state(self, h, qx, qy, w=None, p=None):
+    def set_state(self, h, qx, qy, w=None, p=None, keep_history=False):
         a = [_c64(h, self.cshape), _c64(qx, self.cshape), _c64(qy, self.cshape)]
         b = [None if x is None else _c64(x, self.nshape) for x in (w, p)]
-        self._check(lib().nho_set_state(self._h, *[_ptr(x) for x in a + b]))
+        f = lib().nho_continue_state if keep_history else lib().nho_set_state
+        self._check(f(self._h, *[_ptr(x) for x in a + b]))
 
     def get_state(self):
         h, qx, qy = (np.empty(self.cshape) for _ in range(3))

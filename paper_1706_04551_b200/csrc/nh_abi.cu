@@ -52,7 +52,12 @@ void nh_destroy(nh_ctx* c) {
 int nh_set_state(nh_ctx* c, const double* h, const double* qx, const double* qy, const double* w,
                  const double* p) {
   if (!c) return NH_EINVAL;
-  return NH_FWD(c, nh64::core_set_state(c->c64, h, qx, qy, w, p), nh32::core_set_state(c->c32, h, qx, qy, w, p));
+  return NH_FWD(c, nh64::core_set_state(c->c64, h, qx, qy, w, p, 0), nh32::core_set_state(c->c32, h, qx, qy, w, p, 0));
+}
+int nh_continue_state(nh_ctx* c, const double* h, const double* qx, const double* qy, const double* w,
+                      const double* p) {
+  if (!c) return NH_EINVAL;
+  return NH_FWD(c, nh64::core_set_state(c->c64, h, qx, qy, w, p, 1), nh32::core_set_state(c->c32, h, qx, qy, w, p, 1));
 }
 int nh_get_state(nh_ctx* c, double* h, double* qx, double* qy, double* w, double* p) {
   if (!c) return NH_EINVAL;

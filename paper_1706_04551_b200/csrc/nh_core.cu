@@ -31,15 +31,6 @@ k_all_finite(size_t n, const double* __restrict__ a, int* bad) {
 }
 
 __global__ void k_clear_flag(NhScal* sc, int mask) { sc->flags &= ~mask; }
-// R32: does the p handed to set_state differ anywhere from the most recent solution?
-__global__ void __launch_bounds__(256)
-k_differs(NhGrid G, const real* __restrict__ a, const real* __restrict__ b, int* flag) {
-  int I = blockIdx.x * 32 + threadIdx.x, J = blockIdx.y * 8 + threadIdx.y;
-  bool d = false;
-  if (I < G.nnx && J < G.nny) d = a[(size_t)J * G.np + I] != b[(size_t)J * G.np + I];
-  if (__syncthreads_or(d) && threadIdx.x == 0 && threadIdx.y == 0) atomicOr(flag, 1);
-}
-
 // ---- fp32 variant: the user's arrays are fp64, the planes fp32 (conversion at set / get only) ----
 __global__ void __launch_bounds__(256) k_to_real(size_t n, const double* __restrict__ a, real* __restrict__ b) {
   for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += (size_t)gridDim.x * blockDim.x)
@@ -409,7 +400,7 @@ void core_destroy(Ctx* c) {
 }
 
 int core_set_state(Ctx* c, const double* h, const double* qx, const double* qy, const double* w,
-                 const double* p) {
+                 const double* p, int keep_history) {
   if (!c || !h || !qx || !qy) return NH_EINVAL;
   int s1, s2; other_slots(c->cur, s1, s2);
   // stage into a free slot, validate there, then make it current (an invalid state changes nothing)
@@ -424,24 +415,16 @@ int core_set_state(Ctx* c, const double* h, const double* qx, const double* qy, 
   }
   if (cell_in(c, c->qx[s1], qx) || cell_in(c, c->qy[s1], qy)) return NH_ECUDA;
   nh_launch_validate(c, c->h[s1], c->qx[s1], c->qy[s1]);
-  // p goes through a scratch plane.  R32: when it is bit-identical to the most recent solution the
-  // state is a continuation of the running one (a checkpoint, or a round trip through the host as
-  // in bench.py's end-to-end leg) and the solver's solution history stays valid; any other p
-  // starts a new history.
+  // p goes through a scratch plane (an invalid state must leave the current one untouched)
   if (node_in(c, c->wadv, p)) return NH_ECUDA;
-  const bool maybe_cont = (p != nullptr) && c->nhist > 0;
-  if (cudaMemsetAsync(&c->sc->pad2, 0, sizeof(int), c->stream) != cudaSuccess) { (void)cudaGetLastError(); return NH_ECUDA; }
-  if (maybe_cont) {
-    dim3 blk(32, 8), grd((c->g.nnx + 31) / 32, (c->g.nny + 7) / 8);
-    k_differs<<<grd, blk, 0, c->stream>>>(c->g, c->wadv, c->hist[0], &c->sc->pad2);
-    c->launches++;
-  }
   if (check_launch(c) != NH_OK) return NH_ECUDA;
   if (read_scalars(c) != NH_OK) return NH_ECUDA;
   if (c->sc_host->flags & NH_FLAG_BADSTATE)
     return fail(c, NH_EINVAL, "set_state: h<0 or non-finite input");
   c->cur = s1;
-  if (!(maybe_cont && c->sc_host->pad2 == 0)) c->nhist = 0;
+  // R32: nh_set_state starts a new solution history; nh_continue_state (the caller says that this is
+  // the running state coming back: a checkpoint, a round trip through the host) keeps it
+  if (!keep_history) c->nhist = 0;
   if (node_in(c, c->w[c->curw], w)) return NH_ECUDA;
   if (copy_async(c, c->p - node_origin(c), c->wadv - node_origin(c), c->nni * sizeof(real))) return NH_ECUDA;
   // the CFL rate left by the last RK combine belongs to the replaced state: k_lambda takes a max

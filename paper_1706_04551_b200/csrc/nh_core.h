@@ -13,7 +13,7 @@
                   const nh_params* prm, void* cuda_stream);                                        \
   void core_destroy(Ctx* c);                                                                       \
   int core_set_state(Ctx* c, const double* h, const double* qx, const double* qy, const double* w, \
-                     const double* p);                                                             \
+                     const double* p, int keep_history);                                           \
   int core_get_state(Ctx* c, double* h, double* qx, double* qy, double* w, double* p);            \
   int core_set_time(Ctx* c, double t);                                                             \
   int core_step(Ctx* c, int nsteps);                                                               \

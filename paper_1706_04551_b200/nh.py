@@ -60,7 +60,7 @@ _lib = None
 _vp = C.c_void_p
 
 EXPORTS = (
-    "nh_default_params", "nh_create", "nh_destroy", "nh_set_state", "nh_get_state", "nh_set_time", "nh_step",
+    "nh_default_params", "nh_create", "nh_destroy", "nh_set_state", "nh_continue_state", "nh_get_state", "nh_set_time", "nh_step",
     "nh_hydrostatic_step", "nh_nonhydro_correct", "nh_sync", "nh_get_info", "nh_last_error",
     "nh_launch_count", "nh_profile", "nh_profile_read", "nh_compute_dt", "nh_apply_A", "nh_coeffs",
     "nh_rhs", "nh_constraint", "nh_solve", "nh_breaking", "nh_w_advect", "nh_fp64_rate", "nh_start_vector",
@@ -84,6 +84,7 @@ def lib():
         L.nh_destroy.argtypes = [_vp]
         L.nh_destroy.restype = None
         L.nh_set_state.argtypes = [_vp] * 6
+        L.nh_continue_state.argtypes = [_vp] * 6
         L.nh_get_state.argtypes = [_vp] * 6
         L.nh_set_time.argtypes = [_vp, C.c_double]
         L.nh_step.argtypes = [_vp, C.c_int]
@@ -227,11 +228,14 @@ class NH:
         return st
 
     # ---- state -----------------------------------------------------------------------------
-    def set_state(self, h, qx, qy, w=None, p=None):
+    def set_state(self, h, qx, qy, w=None, p=None, keep_history=False):
+        """nh_set_state (a new run), or with keep_history=True nh_continue_state (the running state
+        coming back: the solver keeps its solution history)."""
         keep = []
         ptrs = [_in(a, self.cshape, keep) for a in (h, qx, qy)] + \
                [_in(a, self.nshape, keep) for a in (w, p)]
-        self._check(lib().nh_set_state(self._h, *ptrs))
+        f = lib().nh_continue_state if keep_history else lib().nh_set_state
+        self._check(f(self._h, *ptrs))
         # pageable host sources are consumed synchronously; device sources are ordered on the stream
 
     def get_state(self, out=None):

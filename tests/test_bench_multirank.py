@@ -66,13 +66,15 @@ def test_reference_arm_rank1_is_silent_and_rank0_prints_one_json_line():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
                         "--steps", "1", "--warmup", "0"], env=env, capture_output=True, text=True, timeout=120)
     assert r.returncode == 0 and r.stdout.strip() == ""
-    env = dict(os.environ, RANK="0", WORLD_SIZE="2", LOCAL_RANK="0", NH_BENCH_ORACLE_CROP="96")
+    env = dict(os.environ, RANK="0", WORLD_SIZE="2", LOCAL_RANK="0")
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
-                        "--steps", "1", "--warmup", "0"], env=env, capture_output=True, text=True, timeout=300)
+                        "--steps", "1", "--warmup", "0", "--oracle-crop", "96"], env=env, capture_output=True,
+                       text=True, timeout=300)
     assert r.returncode == 0, r.stderr
     lines = [l for l in r.stdout.splitlines() if l.strip()]
     assert len(lines) == 1
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+    assert d["config"]["oracle_crop"] == 96 and "96x96" in d["cpu_baseline"]["sample"]
     assert d["unit"] == "cell-updates/s" and d["higher_is_better"] is True

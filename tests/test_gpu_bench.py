@@ -12,9 +12,9 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 def _run(*args, env=None):
-    e = dict(os.environ, NH_BENCH_ORACLE_CROP="96")
+    e = dict(os.environ)
     e.update(env or {})
-    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), *args], capture_output=True, text=True,
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), *args, "--oracle-crop", "96"], capture_output=True, text=True,
                        timeout=900, env=e)
     assert r.returncode == 0, r.stderr[-2000:]
     lines = [l for l in r.stdout.splitlines() if l.strip()]
@@ -37,9 +37,11 @@ def test_bench_line_contract_small_config():
     assert abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and "traffic" in r
     e = d["e2e"]
     assert e["value"] > 0 and e["h2d_bytes_per_step"] == e["d2h_bytes_per_step"] == 8 * (3 * 256 * 192 + 2 * 257 * 193)
-    assert e["value"] < d["value"] * 1.05           # host copies included: not faster than the device leg
+    assert e["value"] < d["value"]                  # same step window + host copies: slower than the device leg
+    assert e["iters_per_solve"] == d["config"]["iters_per_solve"]   # ... and the same solves
     c = d["cpu_baseline"]
-    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["sample"]
+    assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["sample"] and c["iters_per_solve"] > 0
+    assert d["config"]["oracle_crop"] == 96
     assert d["clocks"]["sm_mhz"] and d["clocks"]["sm_max_mhz"] and isinstance(d["clocks"]["reasons"], list)
 
 

@@ -844,8 +844,9 @@ def test_start_vector_saves_iterations_not_accuracy(O, G):
 
 
 def test_set_state_round_trip_keeps_the_solution_history(O, G):
-    # R32: a p bit-identical to the most recent solution marks a continuation (bench.py's end-to-end
-    # leg hands the state back every step): same iteration counts as the uninterrupted run
+    # R32: nh_continue_state hands the running state back (bench.py's end-to-end leg does so every step):
+    # same bits and iteration counts as the uninterrupted run; nh_set_state starts a new history even
+    # when it is given the very same p (the library does not inspect the contents)
     cfg = inputs.make_config(3, nx=200, ny=176)
     a = G.NH(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["H"], **cfg["params"])
     b = G.NH(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["H"], **cfg["params"])
@@ -854,7 +855,7 @@ def test_set_state_round_trip_keeps_the_solution_history(O, G):
         g.step(6)
     for _ in range(4):
         s = b.get_state()
-        b.set_state(s["h"], s["qx"], s["qy"], s["w"], s["p"])
+        b.set_state(s["h"], s["qx"], s["qy"], s["w"], s["p"], keep_history=True)
         assert np.max(np.abs(b.start_vector() - s["p"])) > 0.0
         b.step(1)
         a.step(1)
@@ -864,7 +865,14 @@ def test_set_state_round_trip_keeps_the_solution_history(O, G):
         assert np.array_equal(sa[k], sb[k]), k
     assert a.info().iters_total == b.info().iters_total
     s = b.get_state()
-    p2 = s["p"].copy()
-    p2[5, 7] += 1e-9
-    b.set_state(s["h"], s["qx"], s["qy"], s["w"], p2)
-    assert np.array_equal(b.start_vector(), p2)
+    b.set_state(s["h"], s["qx"], s["qy"], s["w"], s["p"])
+    assert np.array_equal(b.start_vector(), s["p"])
+    # ... and the oracle's two calls behave the same way
+    o = O.Oracle(cfg["nx"], cfg["ny"], cfg["dx"], cfg["dy"], cfg["H"], **cfg["params"])
+    o.set_state(cfg["h"], cfg["qx"], cfg["qy"], cfg["w"], cfg["p"])
+    o.step(8)
+    so = o.get_state()
+    o.set_state(so["h"], so["qx"], so["qy"], so["w"], so["p"], keep_history=True)
+    assert np.max(np.abs(o.start_vector() - so["p"])) > 0.0
+    o.set_state(so["h"], so["qx"], so["qy"], so["w"], so["p"])
+    assert np.array_equal(o.start_vector(), so["p"])

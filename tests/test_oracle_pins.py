@@ -1320,6 +1320,48 @@ def test_start_vector_is_the_quadratic_extrapolation_of_the_solution_increments(
     assert np.array_equal(o.start_vector()[:, :-1], st["p"][:, :-1])
 
 
+def test_start_vector_predicts_the_next_solution_of_a_synthetic_sequence_through_the_library(O):
+    # R32 pinned through the library instead of through its own formula.  With h fixed the operator A
+    # is fixed and the right-hand side b = -B(q, w) / dt (eqs (37)-(40)) is linear in (qx, qy, w): the
+    # states c_k (qx, qy, w) have the solutions s_k = c_k s.  Seven of them are solved one after the
+    # other (continue_state: the same run), with factors whose increments are of two alternating kinds,
+    # each quadratic in k; the start vector of the eighth solve must then BE the eighth solution, c_8 s,
+    # to solver accuracy.  That exercises the rotation of the history, the seven-solution threshold and
+    # every coefficient: changing any one of them misses c_8 s by a multiple of an increment.
+    st = inputs.random_smooth_state(40, 28, 0.3, 0.2, seed=9, depth=1.0, rough=0.3)
+    o = O.Oracle(40, 28, 0.3, 0.2, st["H"], bc_xlo=WALL, bc_xhi=OUT, bc_ylo=WALL, bc_yhi=OUT)
+    k = np.arange(8.0)
+    inc = np.where(k % 2 == 0, 1.0 + 0.3 * k + 0.05 * k * k, -0.2 + 0.1 * k - 0.02 * k * k)
+    c = 2.0 + np.cumsum(inc)                      # c_1 .. c_8
+    sols = []
+    for j in range(7):
+        o.set_state(st["h"], c[j] * st["qx"], c[j] * st["qy"], c[j] * st["w"], None, keep_history=(j > 0))
+        o.nonhydro_correct(0.01)
+        sols.append(o.get_state()["p"].copy())
+        if j < 6:
+            assert np.array_equal(o.start_vector(), sols[-1])      # fewer than seven: the previous solution
+    base = sols[0] / c[0]
+    scale = np.max(np.abs(base))
+    assert scale > 0.0
+    for j in range(7):                                             # the premise: s_k = c_k s
+        assert np.max(np.abs(sols[j] - c[j] * base)) <= 1e-9 * abs(c[j]) * scale
+    x0 = o.start_vector()
+    assert np.max(np.abs(x0 - c[7] * base)) <= 1e-8 * abs(c[7]) * scale
+    assert np.max(np.abs(x0 - sols[-1])) >= 0.5 * abs(c[7] - c[6]) * scale   # not the previous solution
+    # the solve that follows agrees, and starts converged: no iteration beyond the polish
+    o.set_state(st["h"], c[7] * st["qx"], c[7] * st["qy"], c[7] * st["w"], None, keep_history=True)
+    it0 = o.info().iters_total
+    o.nonhydro_correct(0.01)
+    assert np.max(np.abs(o.get_state()["p"] - c[7] * base)) <= 1e-9 * abs(c[7]) * scale
+    assert o.info().iters_total - it0 <= 3
+    # warm_start = 0 is the paper-plain oracle: the same sequence leaves the previous solution
+    o0 = O.Oracle(40, 28, 0.3, 0.2, st["H"], bc_xlo=WALL, bc_xhi=OUT, bc_ylo=WALL, bc_yhi=OUT, warm_start=0)
+    for j in range(7):
+        o0.set_state(st["h"], c[j] * st["qx"], c[j] * st["qy"], c[j] * st["w"], None, keep_history=(j > 0))
+        o0.nonhydro_correct(0.01)
+    assert np.array_equal(o0.start_vector(), o0.get_state()["p"])
+
+
 def test_start_vector_changes_the_iteration_count_not_the_result(O):
     cfg = inputs.make_config(3, nx=96, ny=96)
     out = {}
@@ -1344,14 +1386,14 @@ def test_start_vector_changes_the_iteration_count_not_the_result(O):
 
 
 def test_set_state_keeps_the_solution_history_only_for_a_continuation(O):
-    # R32: handing back the running state (p bit-identical to the most recent solution) keeps the
-    # history -- the run continues exactly as if set_state had not been called; any other p resets it
+    # R32: handing back the running state through continue_state keeps the history -- the run continues
+    # exactly as if the state had never left; set_state (a new run) drops it, whatever p holds
     cfg = inputs.make_config(3, nx=64, ny=64)
     a, b = make(O, cfg), make(O, cfg)
     a.step(6)
     b.step(6)
     s = b.get_state()
-    b.set_state(s["h"], s["qx"], s["qy"], s["w"], s["p"])                 # round trip
+    b.set_state(s["h"], s["qx"], s["qy"], s["w"], s["p"], keep_history=True)   # round trip
     assert np.max(np.abs(b.start_vector() - s["p"])) > 0.0                # still extrapolating
     a.step(3)
     b.step(3)
@@ -1359,9 +1401,8 @@ def test_set_state_keeps_the_solution_history_only_for_a_continuation(O):
     for k in sa:
         assert np.array_equal(sa[k], sb[k]), k
     assert a.info().iters_total == b.info().iters_total
-    p2 = s["p"].copy()
-    p2[5, 7] += 1e-9
-    b.set_state(s["h"], s["qx"], s["qy"], s["w"], p2)                     # a different p: new history
-    assert np.array_equal(b.start_vector(), p2)
+    s = b.get_state()
+    b.set_state(s["h"], s["qx"], s["qy"], s["w"], s["p"])                 # the very same p, but a new run
+    assert np.array_equal(b.start_vector(), s["p"])
     b.set_state(s["h"], s["qx"], s["qy"], s["w"], None)
     assert np.all(b.start_vector() == 0.0)
