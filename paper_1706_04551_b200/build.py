@@ -44,8 +44,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if all(m >= os.path.getmtime(p) for p in _deps()):
             return LIB
     os.makedirs(OBJ, exist_ok=True)
-    extra = os.environ.get("NH_NVCC_EXTRA", "").split()   # developer knob: extra -D switches for experiments
-    common = [_nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-I", INC, "-c"]
+    common = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-I", INC, "-c"]
     jobs = []
     for prec in (64, 32):
         for src in KERNEL_SOURCES:
