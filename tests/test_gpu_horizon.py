@@ -171,3 +171,16 @@ def test_config5_tsunami_crops_200_steps(O, G, window):
     assert g.info().clamps == o.info().clamps
     if window == "coast":
         assert np.any(cfg["h"] == 0.0) and np.any(cfg["h"] > 0.0)     # the shoreline is inside
+
+
+def test_config5_source_crop_1024_twenty_steps(O, G):
+    # a crop of the tsunami basin large enough for the marching warps to run in their full-size shape
+    # (18 strips of 60 columns, bands of many rows, several CTAs per SM busy) and for the Krylov solve to
+    # need hundreds of iterations: 20 whole steps against the oracle at 4 checkpoints, every field at the
+    # north_star bars, qx and qy each against its own maximum
+    cfg = inputs.make_config(5, nx=1024, ny=1024, window="source")
+    o, g, worst = side_by_side(O, G, cfg, 20, ncp=4)
+    assert g.info().clamps == o.info().clamps == 0
+    assert g.info().iters_total > 20 * 2 * 100
+    # the iteration counts of two valid solves of the same systems stay close
+    assert abs(g.info().iters_total - o.info().iters_total) <= 0.05 * o.info().iters_total
