@@ -407,6 +407,47 @@ def run_b200(args):
     return 0
 
 
+def run_streammix(args):
+    """What HBM gives the solver's own read / write mix (nh_stream_mix_rate): planes of the node-plane size of
+    --config, a plain streaming kernel per mix.  One BiCGStab iteration is one pass B (5 planes read, 1 written)
+    plus one pass CA (8 read, 4 written) = 18 planes = 144 B per node: the floor per iteration is the sum of the
+    two passes at the rates their mixes reach, to hold against the ms per iteration bench.py measures.  One
+    JSON line; a record for profiles/, not the driver's bench line."""
+    import torch
+    from paper_1706_04551_b200 import inputs, nh
+    torch.cuda.set_device(0)
+    kw = {}
+    if args.nx:
+        kw["nx"] = args.nx
+    if args.ny:
+        kw["ny"] = args.ny
+    cfg = inputs.make_config(args.config, **kw)
+    nn = (cfg["nx"] + 1) * (cfg["ny"] + 1)
+    n = nn + (nn & 1)
+    peak, peak_src = _peaks()
+    clocks = ClockSampler(0)
+    clocks.start()
+    rates = {}
+    for rep in range(3):          # three rounds: the median per mix
+        for mix in ((1, 1), (5, 1), (8, 4), (6, 1)):
+            rates.setdefault(mix, []).append(nh.stream_mix_rate(mix[0], mix[1], n))
+    clk = clocks.stop()
+    med = {m: float(np.median(v)) for m, v in rates.items()}
+    plane = 8.0 * nn
+    tB, tCA = 6 * plane / (med[(5, 1)] * 1e9), 12 * plane / (med[(8, 4)] * 1e9)
+    print(json.dumps({
+        "streammix": f"{cfg['name']} {cfg['nx']}x{cfg['ny']}", "nodes": nn, "plane_MB": plane / 1e6,
+        "GBs": {f"{m[0]}R+{m[1]}W": med[m] for m in med}, "all_GBs": {f"{m[0]}R+{m[1]}W": v for m, v in rates.items()},
+        "copy_peak_GBs": peak, "peak_source": peak_src,
+        "frac_of_copy_peak": {f"{m[0]}R+{m[1]}W": med[m] / peak for m in med},
+        "bicgstab_floor_ms_per_iteration": 1e3 * (tB + tCA),
+        "bicgstab_floor_note": "pass B (5R+1W, 6 planes) + pass CA (8R+4W, 12 planes) at the rates of their mixes; no "
+                               "halo rows, no grid barrier, no arithmetic",
+        "bicgstab_floor_GBs_at_144B": 144.0 * nn / (tB + tCA) / 1e9,
+        "srj_floor_ms_per_sweep": 1e3 * 7 * plane / (med[(6, 1)] * 1e9), "clocks": clk}))
+    return 0
+
+
 def run_onesolve(args):
     """One pressure solve in isolation, for the ncu capture behind profiles/traffic.json: W warm-up
     steps, then nh_nonhydro_correct(dt_last) = exactly one launch of the solver kernel; prints its
@@ -689,11 +730,15 @@ def main():
                     "configured horizon, parity at 10 checkpoints (slow; a record for profiles/)")
     ap.add_argument("--rtol32", type=float, default=1e-4, help="--precision 32 with --parityruns: solver_rtol of the fp32 run")
     ap.add_argument("--hydrostatic", action="store_true", help="SWE mode (nonhydro = 0): the predictor alone; alu-bound roofline")
+    ap.add_argument("--streammix", action="store_true", help="DRAM rate of plain streaming kernels with the solver's "
+                    "read/write plane mixes on the node-plane size of --config (the floor of an iteration)")
     ap.add_argument("--onesolve", action="store_true", help="one isolated pressure solve after --warmup steps (ncu capture)")
     ap.add_argument("--param", action="append", default=[], help="--parityruns: override a parameter, key=value (repeatable)")
     ap.add_argument("--spread", action="store_true", help="--parityruns: also run a second oracle with a 10 x tighter "
                     "solver tolerance and report oracle-vs-oracle ratios (the spread of two valid solves)")
     args = ap.parse_args()
+    if args.streammix:
+        return run_streammix(args)
     if args.onesolve:
         return run_onesolve(args)
     if args.parityruns:

@@ -205,6 +205,14 @@ int nh_profile_read(nh_ctx* ctx, double* ms, long long* groups);
  * DFMA chains (2 flops each; / 32 = warp instructions as ncu counts them).  Needs no context;
  * synchronises.  dfma_per_second is a HOST pointer. */
 int nh_fp64_rate(void* cuda_stream, double* dfma_per_second);
+/* Measurement hook (bench.py --streammix): the DRAM rate, in GB/s of algorithmic bytes, that a plain
+ * streaming kernel reaches with nread planes read and nwrite planes written per element -- the mix of
+ * one pass of the matrix-free solver (5 + 1 and 8 + 4), of a Jacobi sweep
+ * (6 + 1), or of a copy (1 + 1) -- with ideal access.  Planes of doubles_per_plane doubles (even) are
+ * allocated and freed inside (NH_ENOMEM if they do not fit); other mixes: NH_EINVAL.  Needs no
+ * context; synchronises.  gbytes_per_second is a HOST pointer. */
+int nh_stream_mix_rate(void* cuda_stream, int nread, int nwrite, long long doubles_per_plane,
+                       double* gbytes_per_second);
 
 /* ---- the CFL time step for callers that must not allocate ------------------------------------
  * nh_cfl_dt_static computes dt = cfl / max_ij[(|u|+sqrt(g h))/dx + (|v|+sqrt(g h))/dy] (eq. (23),

@@ -64,7 +64,7 @@ EXPORTS = (
     "nh_hydrostatic_step", "nh_nonhydro_correct", "nh_sync", "nh_get_info", "nh_last_error",
     "nh_launch_count", "nh_profile", "nh_profile_read", "nh_compute_dt", "nh_apply_A", "nh_coeffs",
     "nh_rhs", "nh_constraint", "nh_solve", "nh_breaking", "nh_w_advect", "nh_fp64_rate", "nh_start_vector",
-    "nh_cfl_dt_static", "nh_cfl_dt_static_max_cells", "nh_static_last_error",
+    "nh_cfl_dt_static", "nh_cfl_dt_static_max_cells", "nh_static_last_error", "nh_stream_mix_rate",
 )
 
 
@@ -108,6 +108,7 @@ def lib():
         L.nh_w_advect.argtypes = [_vp, C.c_double, _vp]
         L.nh_start_vector.argtypes = [_vp, _vp]
         L.nh_fp64_rate.argtypes = [_vp, C.POINTER(C.c_double)]
+        L.nh_stream_mix_rate.argtypes = [_vp, C.c_int, C.c_int, C.c_longlong, C.POINTER(C.c_double)]
         L.nh_cfl_dt_static.argtypes = [C.c_int, C.c_int] + [C.c_double] * 5 + [_vp] * 5
         L.nh_cfl_dt_static_max_cells.argtypes = []
         L.nh_cfl_dt_static_max_cells.restype = C.c_longlong
@@ -123,6 +124,16 @@ def fp64_rate(stream=None) -> float:
     st = lib().nh_fp64_rate(None if stream is None else stream.cuda_stream, C.byref(r))
     if st != OK:
         raise NHError(st, "nh_fp64_rate")
+    return r.value
+
+
+def stream_mix_rate(nread, nwrite, doubles_per_plane, stream=None) -> float:
+    """GB/s a plain streaming kernel reaches with `nread` planes read and `nwrite` written (nh_stream_mix_rate)."""
+    r = C.c_double()
+    st = lib().nh_stream_mix_rate(None if stream is None else stream.cuda_stream, int(nread), int(nwrite),
+                                  int(doubles_per_plane), C.byref(r))
+    if st != OK:
+        raise NHError(st, "nh_stream_mix_rate")
     return r.value
 
 

@@ -73,3 +73,16 @@ def test_bench_table2_and_fullruns_modes():
     assert [x["config"] for x in rows] == [1, 2] and all(x["status"] == 0 and x["finite"] for x in rows)
     assert rows[0]["steps"] == 200 and rows[1]["steps"] == 1000 and rows[1]["iters_per_solve"] == 0.0
     assert abs(rows[0]["mass_rel_change"]) < 1e-12 and rows[1]["mass_rel_change"] == 0.0
+
+
+def test_bench_streammix_mode():
+    # the measurement hook behind profiles/r03c: plain streaming kernels with the solver's plane mixes
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--streammix", "--config", "3", "--nx", "1024",
+                        "--ny", "1024"], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    d = json.loads([l for l in r.stdout.splitlines() if l.strip()][-1])
+    assert set(d["GBs"]) == {"1R+1W", "5R+1W", "8R+4W", "6R+1W"} and all(v > 100.0 for v in d["GBs"].values())
+    assert d["nodes"] == 1025 * 1025 and d["bicgstab_floor_ms_per_iteration"] > 0
+    from paper_1706_04551_b200 import nh
+    with pytest.raises(nh.NHError):
+        nh.stream_mix_rate(3, 3, 1024)        # a mix the hook has no kernel for
